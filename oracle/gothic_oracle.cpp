@@ -1,0 +1,459 @@
+/*
+ * gothic_oracle.cpp -- CPU oracle for the GOTHIC hot path (Miki & Umemura, arxiv 1610.07279).
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  It is a plain, slow, step-by-step restatement of what
+ * the paper's method computes, written from PAPER.md (cited as P:<line>) and the readings listed in
+ * DESIGN.md (R1..R12).  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+ * legs may call it.  It shares no code, header, table or helper with the CUDA path under
+ * paper_1610_07279_b200/csrc/, and neither includes the other.
+ *
+ * Build: g++ -O2 -std=c++17 -fopenmp -ffp-contract=off -shared -fPIC   (see oracle/build.py)
+ * -ffp-contract=off matters: every fp32 expression that decides an integer (a key bit, a MAC outcome,
+ * a time-step level) is written with explicit fmaf()/single operations and must not be re-fused.
+ *
+ * Parity pins (tests/test_oracle_*.py, -m "not gpu"):
+ *   direct sum            : eq. 1 vs numpy brute force, two-body closed form, cube symmetry
+ *   encodePeano3D/decode  : bijection, face-adjacency ("one-stroke"), prefix hierarchy,
+ *                           decode(encode) = id, level-1 table from
+ *   Morton                : naive per-bit interleave
+ *   sort                  : permutation / non-decreasing / stable
+ *   tree                  : independent recursive builder + partition invariants
+ *   moments               : numpy brute force (P:62 definitions)
+ *   walk                  : Delta=0 equals eq. 1; error shrinks as Delta tightens;
+ *                           Plummer closed form at large N; momentum
+ *   levels / active set   : closed-form NFW level fractions; nesting invariants
+ * Parity UNPINNED (report only): absolute error-vs-Delta values and interactions per step (the paper
+ * gives them only as figures).
+ */
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <numeric>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef uint64_t PHint; /* "unsigned long int" when the key is longer than 30 bits */
+
+static const int NLEV = 21; /* R1: 21 bits per axis -> 63-bit key */
+
+/* ---- Listing 1, reconstructed: DESIGN.md reading G5 ------------------------------------ */
+static PHint encodePeano3D(int Nlev, PHint px, PHint py, PHint pz)
+{
+    PHint key = 0;
+    for (int jj = Nlev - 1; jj >= 0; jj--) {
+        /* get xi, yi, and zi */
+        PHint xi = (px >> jj) & 1;
+        PHint yi = (py >> jj) & 1;
+        PHint zi = (pz >> jj) & 1;
+        /* turn px, py, and pz */
+        px ^= -(xi & ((!yi) | zi));
+        py ^= -((xi & (yi | zi)) | (yi & (!zi)));
+        pz ^= -((xi & (!yi) & (!zi)) | (yi & (!zi)));
+        /* append 3 bits to the key */
+        key |= ((xi << 2) | ((xi ^ yi) << 1) | ((xi ^ zi) ^ yi)) << (3 * jj);
+        if (zi) { /* rotate uncyclic (x->z->y->x) */
+            PHint pt = px; px = py; py = pz; pz = pt;
+        } else if (!yi) { /* exchange x and z */
+            PHint pt = px; px = pz; pz = pt;
+        }
+    }
+    return key;
+}
+
+/* ---- Listing 2, reconstructed: P:466 prints 3*jj+1 for zi (typo, must be 3*jj);
+ *      the "append 1 bit" lines are lost and re-derived by inverting P:417 ---------------- */
+static void decodePeano3D(int Nlev, PHint key, PHint *rx, PHint *ry, PHint *rz)
+{
+    PHint px = 0, py = 0, pz = 0;
+    for (int jj = 0; jj < Nlev; jj++) {
+        PHint xi = (key >> (3 * jj + 2)) & 1;
+        PHint yi = (key >> (3 * jj + 1)) & 1;
+        PHint zi = (key >> (3 * jj)) & 1;
+        if (yi ^ zi) { /* rotate cyclic (x->y->z->x) */
+            PHint pt = px; px = pz; pz = py; py = pt;
+        } else if (((!xi) & (!yi) & (!zi)) || (xi & yi & zi)) { /* exchange x and z */
+            PHint pt = px; px = pz; pz = pt;
+        }
+        PHint mask = ((PHint)1 << jj) - 1;
+        px ^= mask & (-(xi & (yi | zi)));
+        py ^= mask & (-((xi & ((!yi) | (!zi))) | ((!xi) & yi & zi)));
+        pz ^= mask & (-((xi & (!yi) & (!zi)) | (yi & zi)));
+        px |= xi << jj;          /* append 1 bit to the position: inverse of P:417 */
+        py |= (xi ^ yi) << jj;
+        pz |= (yi ^ zi) << jj;
+    }
+    *rx = px; *ry = py; *rz = pz;
+}
+
+/* ---- Listing 3: Morton key up to 63 bits by multiply-and-mask dilation -------------------- */
+static PHint dilate3D(PHint val)
+{
+    val = (val * 0x100000001ULL) & 0x7fff00000000ffffULL;
+    val = (val * 0x000010001ULL) & 0x00ff0000ff0000ffULL;
+    val = (val * 0x000000101ULL) & 0x700f00f00f00f00fULL;
+    val = (val * 0x000000011ULL) & 0x30c30c30c30c30c3ULL;
+    val = (val * 0x000000005ULL) & 0x1249249249249249ULL;
+    return val;
+}
+static PHint genMorton3D(PHint ix, PHint iy, PHint iz)
+{
+    return (dilate3D(ix) << 2) | (dilate3D(iy) << 1) | dilate3D(iz);
+}
+
+struct Box { float xmin, ymin, zmin, side; };
+
+/* O1 / reading R1: root cube anchored at the per-axis minima, side = smallest power of two strictly
+ * greater than the largest per-axis extent (side = 1 if the extent is 0). */
+static Box root_box(const float *pos_m, uint32_t n)
+{
+    float lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+    for (uint32_t i = 0; i < n; i++)
+        for (int k = 0; k < 3; k++) {
+            float v = pos_m[4 * (size_t)i + k];
+            lo[k] = std::min(lo[k], v);
+            hi[k] = std::max(hi[k], v);
+        }
+    float ext = 0.0f;
+    for (int k = 0; k < 3; k++) ext = std::max(ext, hi[k] - lo[k]);
+    float side = 1.0f;
+    if (ext > 0.0f) {
+        int e;
+        (void)frexpf(ext, &e); /* ext = f * 2^e, f in [0.5, 1)  =>  2^e > ext */
+        side = ldexpf(1.0f, e);
+    }
+    Box b = {lo[0], lo[1], lo[2], side};
+    return b;
+}
+
+/* O2: 21-bit integer coordinate: fp32 subtract, exact power-of-two scaling, truncate, clamp. */
+static inline uint32_t grid_coord(float x, float xmin, float scale)
+{
+    float t = (x - xmin) * scale;
+    float f = floorf(t);
+    if (!(f > 0.0f)) return 0u;
+    if (f >= 2097151.0f) return 2097151u;
+    return (uint32_t)f;
+}
+
+extern "C" {
+
+int oracle_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+uint64_t oracle_encode_peano3d(int nlev, uint64_t x, uint64_t y, uint64_t z) { return encodePeano3D(nlev, x, y, z); }
+void oracle_decode_peano3d(int nlev, uint64_t key, uint64_t *xyz) { decodePeano3D(nlev, key, xyz, xyz + 1, xyz + 2); }
+uint64_t oracle_morton3d(uint64_t x, uint64_t y, uint64_t z) { return genMorton3D(x, y, z); }
+
+void oracle_root_box(const float *pos_m, uint32_t n, float *box4)
+{
+    Box b = root_box(pos_m, n);
+    box4[0] = b.xmin; box4[1] = b.ymin; box4[2] = b.zmin; box4[3] = b.side;
+}
+
+/* O2. key_kind 0 = Peano-Hilbert (paper default), 1 = Morton. */
+void oracle_keys(const float *pos_m, uint32_t n, const float *box4, int key_kind, uint64_t *key)
+{
+    const float scale = 2097152.0f / box4[3];
+    for (uint32_t i = 0; i < n; i++) {
+        uint32_t ix = grid_coord(pos_m[4 * (size_t)i + 0], box4[0], scale);
+        uint32_t iy = grid_coord(pos_m[4 * (size_t)i + 1], box4[1], scale);
+        uint32_t iz = grid_coord(pos_m[4 * (size_t)i + 2], box4[2], scale);
+        key[i] = key_kind == 0 ? encodePeano3D(NLEV, ix, iy, iz) : genMorton3D(ix, iy, iz);
+    }
+}
+
+/* O3: stable sort of (key, original index) by key. */
+void oracle_sort(const uint64_t *key, uint32_t n, uint64_t *key_sorted, uint32_t *perm)
+{
+    std::vector<uint32_t> idx(n);
+    std::iota(idx.begin(), idx.end(), 0u);
+    std::stable_sort(idx.begin(), idx.end(), [&](uint32_t a, uint32_t b) { return key[a] < key[b]; });
+    for (uint32_t s = 0; s < n; s++) { perm[s] = idx[s]; key_sorted[s] = key[idx[s]]; }
+}
+
+/* O4 (reading R2): canonical oct-tree over the sorted keys, breadth-first ids.
+ * Returns the node count, or -1 if it exceeds node_cap.  level_ofs has 23 entries:
+ * level_ofs[L] = id of the first node of level L, level_ofs[n_levels..22] = n_nodes. */
+int64_t oracle_build_tree(const uint64_t *key_sorted, uint32_t n, int n_leaf, uint32_t node_cap,
+                          uint32_t *head, uint32_t *num, uint32_t *child, uint8_t *level, uint8_t *nchild,
+                          uint32_t *level_ofs)
+{
+    struct Nd { uint32_t head, num; };
+    std::vector<Nd> cur, nxt;
+    uint64_t n_nodes = 0;
+    cur.push_back({0u, n});
+    for (int L = 0; L <= NLEV + 1; L++) level_ofs[L] = 0;
+    int L = 0;
+    for (; !cur.empty(); L++) {
+        level_ofs[L] = (uint32_t)n_nodes;
+        const uint64_t base = n_nodes;               /* ids of this level: base .. base+cur.size() */
+        const uint64_t next_base = base + cur.size(); /* ids of the next level start here */
+        if (next_base > node_cap) return -1;
+        nxt.clear();
+        for (size_t k = 0; k < cur.size(); k++) {
+            const uint64_t id = base + k;
+            head[id] = cur[k].head;
+            num[id] = cur[k].num;
+            level[id] = (uint8_t)L;
+            if (cur[k].num > (uint32_t)n_leaf && L < NLEV) {
+                /* children = maximal sub-ranges with equal key >> 3*(21-L-1), in key order;
+                 * empty octants are not stored ("trimTree", Table 2) */
+                const int sh = 3 * (NLEV - L - 1);
+                child[id] = (uint32_t)(next_base + nxt.size());
+                uint32_t s = cur[k].head, e = cur[k].head + cur[k].num, nc = 0;
+                while (s < e) {
+                    uint32_t t = s + 1;
+                    while (t < e && (key_sorted[t] >> sh) == (key_sorted[s] >> sh)) t++;
+                    nxt.push_back({s, t - s});
+                    nc++;
+                    s = t;
+                }
+                nchild[id] = (uint8_t)nc;
+            } else {
+                child[id] = 0xFFFFFFFFu;
+                nchild[id] = 0;
+            }
+        }
+        n_nodes = next_base;
+        cur.swap(nxt);
+    }
+    for (int k = L; k <= NLEV + 1; k++) level_ofs[k] = (uint32_t)n_nodes;
+    return (int64_t)n_nodes;
+}
+
+/* O5 (Fig. 1; reading R9): m_J = sum m_j, r_J = centre of mass, b_J = max |r_j - r_J| measured
+ * from the fp32-rounded r_J that is stored.  Accumulates in double.  Nodes with num = 1 copy the particle. */
+void oracle_moments(const float *pos_sorted, uint32_t n_nodes, const uint32_t *head, const uint32_t *num,
+                    float *com4, float *b)
+{
+#pragma omp parallel for schedule(dynamic, 256)
+    for (int64_t J = 0; J < (int64_t)n_nodes; J++) {
+        const uint32_t h = head[J], c = num[J];
+        if (c == 1) {
+            std::memcpy(com4 + 4 * J, pos_sorted + 4 * (size_t)h, 4 * sizeof(float));
+            b[J] = 0.0f;
+            continue;
+        }
+        double sx = 0, sy = 0, sz = 0, sm = 0;
+        for (uint32_t j = h; j < h + c; j++) {
+            const float *p = pos_sorted + 4 * (size_t)j;
+            sx += (double)p[3] * p[0]; sy += (double)p[3] * p[1]; sz += (double)p[3] * p[2]; sm += p[3];
+        }
+        const float cx = (float)(sx / sm), cy = (float)(sy / sm), cz = (float)(sz / sm);
+        double b2 = 0.0;
+        for (uint32_t j = h; j < h + c; j++) {
+            const float *p = pos_sorted + 4 * (size_t)j;
+            const double dx = (double)p[0] - cx, dy = (double)p[1] - cy, dz = (double)p[2] - cz;
+            b2 = std::max(b2, dx * dx + dy * dy + dz * dz);
+        }
+        com4[4 * J + 0] = cx; com4[4 * J + 1] = cy; com4[4 * J + 2] = cz; com4[4 * J + 3] = (float)sm;
+        b[J] = (float)std::sqrt(b2);
+    }
+}
+
+/* O6 (reading R6; criterion from BASELINE.json configs[2]): dt_i = eta sqrt(eps/|a_i|) floored to a power
+ * of two.  q = dt^4 = c / |a|^2 with c = (float)(eta^4 eps^2) formed by the caller; exponent of dt =
+ * floor(ilogb(q) / 4).  Levels count up from the finest present, clamped to max_levels - 1. */
+static inline int dt_exponent(const float *a, float c)
+{
+    const float a2 = fmaf(a[2], a[2], fmaf(a[1], a[1], a[0] * a[0]));
+    if (!(a2 > 0.0f)) return 127;          /* |a| = 0 (or NaN): coarsest */
+    const float q = c / a2;
+    if (std::isinf(q) || std::isnan(q)) return 127;
+    if (q == 0.0f) return -38;             /* below the smallest subnormal: floor(-150/4) */
+    const int e = ilogbf(q);               /* exact integer exponent, subnormals included */
+    return (e >= 0) ? e / 4 : -((-e + 3) / 4); /* floor division */
+}
+
+void oracle_levels(const float *acc_pot, uint32_t n, float c, int max_levels, uint8_t *level, int32_t *emin_nlev)
+{
+    int emin = 1 << 30;
+    std::vector<int> e(n);
+    for (uint32_t i = 0; i < n; i++) { e[i] = dt_exponent(acc_pot + 4 * (size_t)i, c); emin = std::min(emin, e[i]); }
+    int lmax = 0;
+    for (uint32_t i = 0; i < n; i++) {
+        int l = std::min(e[i] - emin, max_levels - 1);
+        level[i] = (uint8_t)l;
+        lmax = std::max(lmax, l);
+    }
+    emin_nlev[0] = n ? emin : 0;
+    emin_nlev[1] = n ? lmax + 1 : 0;
+}
+
+/* O6: particle active at substep s (1-based) iff s mod 2^level == 0  <=>  level <= ctz(s). */
+uint32_t oracle_active(const uint8_t *level, uint32_t n, uint32_t substep, uint32_t *active)
+{
+    uint32_t k = 0;
+    for (uint32_t i = 0; i < n; i++) {
+        const uint32_t period = 1u << level[i];
+        if (substep % period == 0) active[k++] = i;
+    }
+    return k;
+}
+
+/* Eq. 1 in double, G = 1, with the potential of reading R5:
+ * a_i = sum_{j != i} m_j (r_j - r_i) / (|r_j - r_i|^2 + eps^2)^{3/2},  Phi_i = - sum_{j != i} m_j / sqrt(...).
+ * targets == NULL -> all particles.  out4: (ax, ay, az, Phi) per target. */
+void oracle_direct(const float *pos_m, uint32_t n, const uint32_t *targets, uint32_t nt, double eps, double *out4)
+{
+    const double eps2 = eps * eps;
+    const uint32_t m = targets ? nt : n;
+#pragma omp parallel for schedule(static)
+    for (int64_t t = 0; t < (int64_t)m; t++) {
+        const uint32_t i = targets ? targets[t] : (uint32_t)t;
+        const double xi = pos_m[4 * (size_t)i], yi = pos_m[4 * (size_t)i + 1], zi = pos_m[4 * (size_t)i + 2];
+        double ax = 0, ay = 0, az = 0, ph = 0;
+        for (uint32_t j = 0; j < n; j++) {
+            if (j == i) continue;
+            const double dx = pos_m[4 * (size_t)j] - xi, dy = pos_m[4 * (size_t)j + 1] - yi, dz = pos_m[4 * (size_t)j + 2] - zi;
+            const double r2 = dx * dx + dy * dy + dz * dz + eps2;
+            const double u = 1.0 / std::sqrt(r2);
+            const double mu3 = pos_m[4 * (size_t)j + 3] * u * u * u;
+            ax += mu3 * dx; ay += mu3 * dy; az += mu3 * dz;
+            ph -= pos_m[4 * (size_t)j + 3] * u;
+        }
+        out4[4 * t] = ax; out4[4 * t + 1] = ay; out4[4 * t + 2] = az; out4[4 * t + 3] = ph;
+    }
+}
+
+/* O7 (P:105-118 traversal with a pseudo i-particle; eq. 5; eq. 2; P:62 monopole).
+ * One group = aligned chunk of G consecutive sorted indices (reading R3); members = its active particles;
+ * GEO enclosing ball and a_min = min |a_old| over members (R4).  All MAC-deciding arithmetic in fp32 with
+ * the operation order written here; the sums over the interaction list are in double.
+ *   active == NULL  -> all n particles active.
+ *   out4: double (ax, ay, az, Phi) for every sorted index (only active entries written).
+ *   counts[0] += sum over groups |K| * |list|   (interactions, P:331 convention)
+ *   counts[1] += MAC evaluations, counts[2] += groups walked, counts[3] += sum |list|
+ *   group_lo/group_hi: only groups g with group_lo <= g < group_hi are walked (bounded samples). */
+void oracle_walk(const float *pos_sorted, uint32_t n,
+                 const uint32_t *head, const uint32_t *num, const uint32_t *child, const uint8_t *nchild,
+                 const float *com4, const float *bJ,
+                 const uint32_t *active, uint32_t n_active, int G,
+                 float eps, int mac_kind, float mac_param, const float *aold,
+                 uint32_t group_lo, uint32_t group_hi,
+                 double *out4, uint64_t *counts)
+{
+    const uint32_t n_groups = (n + (uint32_t)G - 1) / (uint32_t)G;
+    group_hi = std::min(group_hi, n_groups);
+    /* members per group from the ascending active list */
+    std::vector<uint32_t> first(n_groups + 1, 0);
+    if (active) {
+        for (uint32_t k = 0; k < n_active; k++) first[active[k] / G + 1]++;
+        for (uint32_t g = 0; g < n_groups; g++) first[g + 1] += first[g];
+    }
+    const double eps2 = (double)eps * (double)eps;
+    uint64_t c_int = 0, c_mac = 0, c_grp = 0, c_list = 0;
+
+#pragma omp parallel for schedule(dynamic, 16) reduction(+ : c_int, c_mac, c_grp, c_list)
+    for (int64_t g = group_lo; g < (int64_t)group_hi; g++) {
+        std::vector<uint32_t> K;
+        if (active) {
+            for (uint32_t k = first[g]; k < first[g + 1]; k++) K.push_back(active[k]);
+        } else {
+            for (uint32_t s = (uint32_t)g * G; s < std::min(n, (uint32_t)(g + 1) * G); s++) K.push_back(s);
+        }
+        if (K.empty()) continue;
+        /* pseudo i-particle: GEO ball (App. B P:568 item 3) */
+        float lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+        float amin = INFINITY;
+        for (uint32_t k : K) {
+            for (int d = 0; d < 3; d++) {
+                lo[d] = std::min(lo[d], pos_sorted[4 * (size_t)k + d]);
+                hi[d] = std::max(hi[d], pos_sorted[4 * (size_t)k + d]);
+            }
+            if (aold) amin = std::min(amin, aold[k]);
+        }
+        float rI[3];
+        for (int d = 0; d < 3; d++) rI[d] = 0.5f * (lo[d] + hi[d]);
+        float b2max = 0.0f;
+        for (uint32_t k : K) {
+            const float dx = pos_sorted[4 * (size_t)k] - rI[0], dy = pos_sorted[4 * (size_t)k + 1] - rI[1],
+                        dz = pos_sorted[4 * (size_t)k + 2] - rI[2];
+            b2max = std::max(b2max, fmaf(dz, dz, fmaf(dy, dy, dx * dx)));
+        }
+        const float bI = sqrtf(b2max);
+        const float thr = mac_kind == 0 ? mac_param * amin : mac_param; /* Delta_acc * a_min (G = 1), or theta */
+
+        /* traversal: pending set handled as a stack ("any order", R10) */
+        std::vector<uint32_t> pending(1, 0u);
+        std::vector<uint32_t> cells, parts; /* accepted cells; particles of opened leaves */
+        while (!pending.empty()) {
+            const uint32_t J = pending.back();
+            pending.pop_back();
+            c_mac++;
+            const float dx = com4[4 * (size_t)J] - rI[0], dy = com4[4 * (size_t)J + 1] - rI[1], dz = com4[4 * (size_t)J + 2] - rI[2];
+            const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+            const float d = fmaxf(sqrtf(r2) - bI, 0.0f); /* eq. 6-7: lambda * r_JI */
+            bool accept = false;
+            if (d > 0.0f) {
+                if (mac_kind == 0) {
+                    const float mb2 = (com4[4 * (size_t)J + 3] * bJ[J]) * bJ[J];
+                    accept = thr * ((d * d) * (d * d)) >= mb2; /* eq. 5, both sides to the 4th power */
+                } else {
+                    accept = bJ[J] <= thr * d;                 /* eq. 2 */
+                }
+            }
+            if (accept) cells.push_back(J);
+            else if (child[J] == 0xFFFFFFFFu) {
+                for (uint32_t s = head[J]; s < head[J] + num[J]; s++) parts.push_back(s);
+            } else {
+                for (uint32_t c = 0; c < nchild[J]; c++) pending.push_back(child[J] + c);
+            }
+        }
+        /* evaluate: every member against every list entry (eq. 1 with pseudo j-particles, monopole) */
+        for (uint32_t i : K) {
+            const double xi = pos_sorted[4 * (size_t)i], yi = pos_sorted[4 * (size_t)i + 1], zi = pos_sorted[4 * (size_t)i + 2];
+            double ax = 0, ay = 0, az = 0, ph = 0;
+            for (uint32_t J : cells) {
+                const double dx = com4[4 * (size_t)J] - xi, dy = com4[4 * (size_t)J + 1] - yi, dz = com4[4 * (size_t)J + 2] - zi;
+                const double u = 1.0 / std::sqrt(dx * dx + dy * dy + dz * dz + eps2);
+                const double mu3 = com4[4 * (size_t)J + 3] * u * u * u;
+                ax += mu3 * dx; ay += mu3 * dy; az += mu3 * dz; ph -= com4[4 * (size_t)J + 3] * u;
+            }
+            for (uint32_t s : parts) {
+                if (s == i) continue; /* j != i (eq. 1); reading R5 */
+                const double dx = pos_sorted[4 * (size_t)s] - xi, dy = pos_sorted[4 * (size_t)s + 1] - yi, dz = pos_sorted[4 * (size_t)s + 2] - zi;
+                const double u = 1.0 / std::sqrt(dx * dx + dy * dy + dz * dz + eps2);
+                const double mu3 = pos_sorted[4 * (size_t)s + 3] * u * u * u;
+                ax += mu3 * dx; ay += mu3 * dy; az += mu3 * dz; ph -= pos_sorted[4 * (size_t)s + 3] * u;
+            }
+            out4[4 * (size_t)i] = ax; out4[4 * (size_t)i + 1] = ay; out4[4 * (size_t)i + 2] = az; out4[4 * (size_t)i + 3] = ph;
+        }
+        const uint64_t L = cells.size() + parts.size();
+        c_int += (uint64_t)K.size() * L;
+        c_list += L;
+        c_grp++;
+    }
+    if (counts) { counts[0] += c_int; counts[1] += c_mac; counts[2] += c_grp; counts[3] += c_list; }
+}
+
+/* P:118 pin helper: for one group, the ball (r_I, b_I) exactly as oracle_walk forms it. */
+void oracle_group_ball(const float *pos_sorted, const uint32_t *members, uint32_t k, float *ball4)
+{
+    float lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+    for (uint32_t q = 0; q < k; q++)
+        for (int d = 0; d < 3; d++) {
+            lo[d] = std::min(lo[d], pos_sorted[4 * (size_t)members[q] + d]);
+            hi[d] = std::max(hi[d], pos_sorted[4 * (size_t)members[q] + d]);
+        }
+    float rI[3];
+    for (int d = 0; d < 3; d++) rI[d] = 0.5f * (lo[d] + hi[d]);
+    float b2max = 0.0f;
+    for (uint32_t q = 0; q < k; q++) {
+        const float dx = pos_sorted[4 * (size_t)members[q]] - rI[0], dy = pos_sorted[4 * (size_t)members[q] + 1] - rI[1],
+                    dz = pos_sorted[4 * (size_t)members[q] + 2] - rI[2];
+        b2max = std::max(b2max, fmaf(dz, dz, fmaf(dy, dy, dx * dx)));
+    }
+    ball4[0] = rI[0]; ball4[1] = rI[1]; ball4[2] = rI[2]; ball4[3] = sqrtf(b2max);
+}
+
+} /* extern "C" */

@@ -1,0 +1,176 @@
+"""Seeded synthetic particle models (the five BASELINE.json configs).
+
+This module is the ONLY code shared by the CUDA path's tests/bench and the CPU oracle's tests.
+It holds none of the method's arithmetic (no keys, no tree, no forces): it only draws positions
+and masses.  The paper's own initial conditions came from the MAGI generator, which
+is not available; these seed-driven spheres and the composite disk model stand in for them
+(recipe: DESIGN.md "Input recipe").
+
+All models: G = 1, total mass 1, equal masses 1/N, float64 maths -> float32 (x, y, z, m) rows.
+Radii are drawn by inverse CDF of the TRUNCATED profile, directions isotropic.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+__all__ = [
+    "plummer", "hernquist", "nfw", "m31_like", "make_config", "CONFIGS", "random_active_subset",
+]
+
+
+def _rng(seed: int) -> np.random.Generator:
+    return np.random.Generator(np.random.PCG64(int(seed)))
+
+
+def _isotropic(rng: np.random.Generator, r: np.ndarray) -> np.ndarray:
+    n = r.shape[0]
+    cth = rng.uniform(-1.0, 1.0, n)
+    phi = rng.uniform(0.0, 2.0 * np.pi, n)
+    sth = np.sqrt(np.maximum(0.0, 1.0 - cth * cth))
+    return np.stack([r * sth * np.cos(phi), r * sth * np.sin(phi), r * cth], axis=1)
+
+
+def _open_uniform(rng: np.random.Generator, n: int, hi: float) -> np.ndarray:
+    """u in (0, hi): strictly inside so that inverse CDFs stay finite."""
+    u = rng.uniform(0.0, 1.0, n)
+    u = np.clip(u, 1e-15, 1.0 - 1e-15)
+    return u * hi
+
+
+def _r_plummer(rng, n, a=1.0, rmax=20.0):
+    x = rmax / a
+    m_r = x ** 3 / (1.0 + x * x) ** 1.5
+    u = _open_uniform(rng, n, m_r)
+    return a / np.sqrt(u ** (-2.0 / 3.0) - 1.0)
+
+
+def _r_hernquist(rng, n, a=1.0, rmax=100.0):
+    x = rmax / a
+    m_r = (x / (1.0 + x)) ** 2
+    s = np.sqrt(_open_uniform(rng, n, m_r))
+    return a * s / (1.0 - s)
+
+
+def _nfw_mu(x):
+    return np.log1p(x) - x / (1.0 + x)
+
+
+def _r_nfw(rng, n, rs=1.0, rmax=10.0):
+    xmax = rmax / rs
+    target = _open_uniform(rng, n, float(_nfw_mu(xmax)))
+    lo = np.zeros(n)
+    hi = np.full(n, xmax)
+    # bisection in float64: mu is monotone on [0, xmax]; 60 halvings reach double precision
+    for _ in range(60):
+        mid = 0.5 * (lo + hi)
+        below = _nfw_mu(mid) < target
+        lo = np.where(below, mid, lo)
+        hi = np.where(below, hi, mid)
+    return rs * 0.5 * (lo + hi)
+
+
+def _disk(rng, n, rd=1.0, zd=0.1, rmax=10.0):
+    """Exponential surface density (R ~ Gamma(2, rd), truncated at rmax by rejection), sech^2 in z."""
+    out_r = np.empty(n)
+    filled = 0
+    while filled < n:
+        m = n - filled
+        u1 = np.clip(rng.uniform(0.0, 1.0, m), 1e-300, 1.0)
+        u2 = np.clip(rng.uniform(0.0, 1.0, m), 1e-300, 1.0)
+        r = -rd * np.log(u1 * u2)
+        r = r[r <= rmax]
+        out_r[filled:filled + r.shape[0]] = r
+        filled += r.shape[0]
+    phi = rng.uniform(0.0, 2.0 * np.pi, n)
+    u = np.clip(rng.uniform(0.0, 1.0, n), 1e-15, 1.0 - 1e-15)
+    z = zd * np.arctanh(2.0 * u - 1.0)
+    return np.stack([out_r * np.cos(phi), out_r * np.sin(phi), z], axis=1)
+
+
+def _finish(rng: np.random.Generator, xyz64: np.ndarray) -> np.ndarray:
+    """Cast to fp32, give every particle mass 1/N, and re-draw exact duplicate positions
+    (shifted by a few fp32 ulps) so that no two particles coincide."""
+    n = xyz64.shape[0]
+    out = np.empty((n, 4), dtype=np.float32)
+    out[:, :3] = xyz64.astype(np.float32)
+    out[:, 3] = np.float32(1.0 / n)
+    for _ in range(8):
+        bits = out[:, :3].view(np.uint32).astype(np.uint64)
+        h = (bits[:, 0] * np.uint64(0x9E3779B97F4A7C15)) ^ (bits[:, 1] * np.uint64(0xC2B2AE3D27D4EB4F)) \
+            ^ (bits[:, 2] * np.uint64(0x165667B19E3779F9))
+        order = np.argsort(h, kind="stable")
+        hs = h[order]
+        cand = np.nonzero(hs[1:] == hs[:-1])[0]
+        if cand.size == 0:
+            break
+        a, b = order[cand], order[cand + 1]
+        same = np.all(out[a, :3] == out[b, :3], axis=1)
+        dup = b[same]
+        if dup.size == 0:
+            break
+        jitter = rng.integers(1, 64, size=(dup.size, 3)).astype(np.float32)
+        out[dup, :3] = out[dup, :3] + jitter * np.spacing(np.abs(out[dup, :3]) + np.float32(1e-30))
+    return out
+
+
+def plummer(n: int, seed: int = 1, a: float = 1.0, rmax: float = 20.0) -> np.ndarray:
+    rng = _rng(seed)
+    return _finish(rng, _isotropic(rng, _r_plummer(rng, n, a, rmax)))
+
+
+def hernquist(n: int, seed: int = 1, a: float = 1.0, rmax: float = 100.0) -> np.ndarray:
+    rng = _rng(seed)
+    return _finish(rng, _isotropic(rng, _r_hernquist(rng, n, a, rmax)))
+
+
+def nfw(n: int, seed: int = 1, rs: float = 1.0, rmax: float = 10.0) -> np.ndarray:
+    rng = _rng(seed)
+    return _finish(rng, _isotropic(rng, _r_nfw(rng, n, rs, rmax)))
+
+
+def m31_like(n: int, seed: int = 1) -> np.ndarray:
+    """NFW halo 81 % + Hernquist bulge 8 % + exponential disk 11 % by mass (BASELINE.json configs[3]);
+    equal-mass particles, so the split is by count.  Scale radii in units of R_d = 1:
+    halo r_s = 1.413 (cut at 10 r_s), bulge a = 0.113 (cut at 100 a), disk R_d = 1, z_d = 0.1."""
+    rng = _rng(seed)
+    n_bulge = int(round(0.08 * n))
+    n_disk = int(round(0.11 * n))
+    n_halo = n - n_bulge - n_disk
+    halo = _isotropic(rng, _r_nfw(rng, n_halo, 1.413, 14.13))
+    bulge = _isotropic(rng, _r_hernquist(rng, n_bulge, 0.113, 11.3))
+    disk = _disk(rng, n_disk, 1.0, 0.1, 10.0)
+    xyz = np.concatenate([halo, bulge, disk], axis=0)
+    xyz = xyz[rng.permutation(n)]
+    return _finish(rng, xyz)
+
+
+def random_active_subset(n: int, fraction: float, seed: int = 7) -> np.ndarray:
+    """Ascending uint32 indices of a random subset (BASELINE.json configs[4], fixed seed)."""
+    rng = _rng(seed)
+    k = max(1, int(round(fraction * n)))
+    if k >= n:
+        return np.arange(n, dtype=np.uint32)
+    idx = rng.choice(n, size=k, replace=False)
+    idx.sort()
+    return idx.astype(np.uint32)
+
+
+# name -> (generator, N, eps, delta_acc, description) : BASELINE.json "configs" in order
+CONFIGS = {
+    "plummer_2p13": dict(model=plummer, n=1 << 13, eps=1.0 / 64, delta_acc=2.0 ** -7, block=False),
+    "hernquist_2p20": dict(model=hernquist, n=1 << 20, eps=2.0 ** -7, delta_acc=2.0 ** -9, block=False),
+    "nfw_2p24_block": dict(model=nfw, n=1 << 24, eps=2.0 ** -8, delta_acc=2.0 ** -9, block=True),
+    "m31_2p24_block": dict(model=m31_like, n=1 << 24, eps=2.0 ** -8, delta_acc=2.0 ** -9, block=True),
+    "nfw_2p22_sweep": dict(model=nfw, n=1 << 22, eps=2.0 ** -8, delta_acc=2.0 ** -9, block=False),
+}
+
+
+def make_config(name: str, seed: int = 1, n: int | None = None) -> tuple[np.ndarray, dict]:
+    """Returns (pos_m float32 [N,4], parameters).  `n` overrides N (smaller parity-test sizes)."""
+    cfg = dict(CONFIGS[name])
+    if n is not None:
+        cfg["n"] = int(n)
+    pos = cfg["model"](cfg["n"], seed)
+    cfg["name"] = name
+    cfg["seed"] = seed
+    return pos, cfg

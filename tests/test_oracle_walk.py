@@ -1,0 +1,159 @@
+"""Pins for the oracle's direct sum (eq. 1) and group tree walk (O7: eq. 5-7)."""
+import numpy as np
+import pytest
+
+from paper_1610_07279_b200 import workloads as W
+
+
+def _brute_numpy(pos, eps):
+    p = pos.astype(np.float64)
+    d = p[None, :, :3] - p[:, None, :3]
+    r2 = (d ** 2).sum(-1) + eps * eps
+    np.fill_diagonal(r2, np.inf)
+    u = 1.0 / np.sqrt(r2)
+    acc = (p[None, :, 3:4] * u[..., None] ** 3 * d).sum(1)
+    pot = -(p[None, :, 3] * u).sum(1)
+    return np.concatenate([acc, pot[:, None]], axis=1)
+
+
+def test_direct_matches_numpy_bruteforce(oracle):
+    rng = np.random.default_rng(1)
+    pos = W.plummer(300, seed=3)
+    pos[:, 3] = rng.uniform(0.1, 2.0, 300).astype(np.float32)
+    ref = _brute_numpy(pos, 0.05)
+    out = oracle.direct(pos, 0.05)
+    assert np.allclose(out, ref, rtol=1e-12, atol=1e-13)
+    sub = np.array([5, 17, 299], np.uint32)
+    assert np.allclose(oracle.direct(pos, 0.05, sub), ref[sub], rtol=1e-12, atol=1e-13)
+
+
+def test_two_body_closed_form(oracle):
+    """Textbook: two softened point masses on the x axis."""
+    m1, m2, d, eps = 2.0, 3.0, 1.5, 0.25
+    pos = np.array([[0, 0, 0, m1], [d, 0, 0, m2]], np.float32)
+    out = oracle.direct(pos, eps)
+    s = (d * d + eps * eps)
+    assert out[0] == pytest.approx([m2 * d / s ** 1.5, 0, 0, -m2 / s ** 0.5], rel=1e-12)
+    assert out[1] == pytest.approx([-m1 * d / s ** 1.5, 0, 0, -m1 / s ** 0.5], rel=1e-12)
+
+
+def test_cube_corner_symmetry(oracle):
+    """8 equal masses on cube corners: |a| equal, pointing at the centre; a test mass at the centre feels 0."""
+    c = np.array([[x, y, z] for x in (-1, 1) for y in (-1, 1) for z in (-1, 1)], np.float32)
+    pos = np.concatenate([np.c_[c, np.ones(8, np.float32)], [[0, 0, 0, 1e-3]]]).astype(np.float32)
+    out = oracle.direct(pos, 0.1)
+    assert np.allclose(out[8, :3], 0, atol=1e-14)
+    a = out[:8, :3]
+    mag = np.linalg.norm(a, axis=1)
+    assert np.allclose(mag, mag[0], rtol=1e-12)
+    assert np.allclose(a / mag[:, None], -c / np.sqrt(3), atol=1e-12)
+
+
+@pytest.mark.parametrize("n,active_frac,G", [(1500, 1.0, 32), (1500, 0.2, 32), (777, 1.0, 16), (40, 1.0, 32)])
+def test_walk_with_nothing_accepted_equals_direct(oracle, n, active_frac, G):
+    """Delta_acc = 0 / theta = 0: no cell is ever accepted, the list is all particles => eq. 1."""
+    pos = W.hernquist(n, seed=5)
+    t = oracle.build_tree(pos, n_leaf=8)
+    eps = float(np.float32(0.01))  # the walk takes eps as fp32: give eq. 1 the same value
+    ref = oracle.direct(t.pos_sorted, eps)
+    active = None if active_frac == 1.0 else W.random_active_subset(n, active_frac)
+    rows = np.arange(n) if active is None else active
+    for kind, aold in ((1, None), (0, np.ones(n, np.float32))):
+        out, cnt = oracle.walk_tree(t, eps=eps, mac_kind=kind, mac_param=0.0, aold=aold, active=active, group_size=G)
+        assert np.allclose(out[rows], ref[rows], rtol=1e-11, atol=1e-13)
+        assert cnt["interactions"] == len(rows) * n
+        if active is not None:
+            mask = np.ones(n, bool)
+            mask[active] = False
+            assert np.all(out[mask] == 0)  # only active entries written
+
+
+def test_pseudo_i_distance_is_conservative(oracle):
+    """the ball-surface distance never exceeds the true distance of any member to the pseudo-j."""
+    pos = W.plummer(4096, seed=8)
+    t = oracle.build_tree(pos)
+    rng = np.random.default_rng(0)
+    p = t.pos_sorted.astype(np.float64)
+    for g in range(0, 128, 3):
+        members = np.arange(32 * g, 32 * g + 32, dtype=np.uint32)
+        members = members[rng.random(32) < 0.6]
+        if members.size == 0:
+            continue
+        ball = oracle.group_ball(t.pos_sorted, members).astype(np.float64)
+        rk = np.linalg.norm(p[members, :3] - ball[:3], axis=1)
+        assert np.all(rk <= ball[3] * (1 + 1e-6))
+        for J in rng.integers(0, t.n_nodes, 50):
+            rJ = t.com[J, :3].astype(np.float64)
+            d = max(np.linalg.norm(rJ - ball[:3]) - ball[3], 0.0)
+            assert d <= np.linalg.norm(p[members, :3] - rJ, axis=1).min() * (1 + 1e-6) + 1e-7
+
+
+@pytest.fixture(scope="module")
+def plummer_case(oracle):
+    pos, cfg = W.make_config("plummer_2p13", seed=1)
+    t = oracle.build_tree(pos)
+    ref = oracle.direct(t.pos_sorted, cfg["eps"])
+    boot, _ = oracle.walk_tree(t, eps=cfg["eps"], mac_kind=1, mac_param=0.5)
+    aold = np.linalg.norm(boot[:, :3], axis=1).astype(np.float32)
+    return t, cfg, ref, aold
+
+
+def _rel_err(out, ref):
+    return np.linalg.norm(out[:, :3] - ref[:, :3], axis=1) / np.linalg.norm(ref[:, :3], axis=1)
+
+
+def test_error_shrinks_as_accuracy_parameter_tightens(oracle, plummer_case):
+    """tighter Delta_acc => smaller error; ~1e-3 median for Delta_acc 2^-8..2^-6."""
+    t, cfg, ref, aold = plummer_case
+    med, p99, work, mom = [], [], [], []
+    for ld in (1, 3, 5, 7, 9, 11, 14, 17, 20):
+        out, cnt = oracle.walk_tree(t, eps=cfg["eps"], mac_kind=0, mac_param=2.0 ** -ld, aold=aold)
+        e = _rel_err(out, ref)
+        med.append(np.median(e)); p99.append(np.percentile(e, 99)); work.append(cnt["interactions"])
+        m = t.pos_sorted[:, 3:4].astype(np.float64)
+        mom.append(np.linalg.norm((m * out[:, :3]).sum(0)) / (m[:, 0] * np.linalg.norm(out[:, :3], axis=1)).sum())
+    assert all(a > b for a, b in zip(med, med[1:])) and all(a > b for a, b in zip(p99, p99[1:]))
+    assert all(a < b for a, b in zip(work, work[1:]))
+    assert 3e-4 < med[3] < 3e-3            # Delta_acc = 2^-7
+    assert med[-1] < 1e-5
+    assert mom[-1] < mom[0] and mom[3] < 3 * med[3]   # momentum near-conservation tracks the force error
+    # opening angle eq. 2 as well: theta 0.9 -> 0.3 monotone
+    e_t = [np.median(_rel_err(oracle.walk_tree(t, eps=cfg["eps"], mac_kind=1, mac_param=th)[0], ref)) for th in (0.9, 0.6, 0.3)]
+    assert e_t[0] > e_t[1] > e_t[2]
+
+
+def test_potential_matches_direct(oracle, plummer_case):
+    t, cfg, ref, aold = plummer_case
+    out, _ = oracle.walk_tree(t, eps=cfg["eps"], mac_kind=0, mac_param=2.0 ** -9, aold=aold)
+    assert np.median(np.abs(out[:, 3] - ref[:, 3]) / np.abs(ref[:, 3])) < 2e-4
+    assert np.all(out[:, 3] < 0)
+
+
+def test_plummer_closed_form_large_n(oracle):
+    """Exact Plummer sphere (a = 1, truncated at R = 20, mass renormalised to 1):
+    M(<r) = r^3/(1+r^2)^{3/2} / M_R,  a_r = -M(<r)/r^2,  Phi(r) = -[(1+r^2)^{-1/2} - (1+R^2)^{-3/2} ... ]
+    Here the potential is checked through Phi(r) = -M(<r)/r - int_r^R dM/r' computed by quadrature of the
+    closed-form density, the radial acceleration through M(<r)."""
+    n = 1 << 15
+    pos = W.plummer(n, seed=2)
+    eps = 1.0 / 64
+    t = oracle.build_tree(pos)
+    boot, _ = oracle.walk_tree(t, eps=eps, mac_kind=1, mac_param=0.5)
+    aold = np.linalg.norm(boot[:, :3], axis=1).astype(np.float32)
+    out, _ = oracle.walk_tree(t, eps=eps, mac_kind=0, mac_param=2.0 ** -9, aold=aold)
+    p = t.pos_sorted.astype(np.float64)
+    r = np.linalg.norm(p[:, :3], axis=1)
+    a_r = (out[:, :3] * p[:, :3]).sum(1) / r
+    R = 20.0
+    MR = R ** 3 / (1 + R * R) ** 1.5
+    mass = lambda x: x ** 3 / (1 + x * x) ** 1.5 / MR
+    # Phi(r) = -M(<r)/r - int_r^R (dM/dr')/r' dr' ; dM/dr = 3 r^2 (1+r^2)^{-5/2}/MR ; integral closed form:
+    # int 3 r (1+r^2)^{-5/2} dr = -(1+r^2)^{-3/2}
+    phi = lambda x: -mass(x) / x - ((1 + x * x) ** -1.5 - (1 + R * R) ** -1.5) / MR
+    edges = np.geomspace(0.2, 8.0, 13)
+    for lo, hi in zip(edges[:-1], edges[1:]):
+        sel = (r >= lo) & (r < hi)
+        k = sel.sum()
+        assert k > 300
+        assert np.mean(a_r[sel]) == pytest.approx(np.mean(-mass(r[sel]) / r[sel] ** 2), rel=6.0 / np.sqrt(k))
+        assert np.mean(out[sel, 3]) == pytest.approx(np.mean(phi(r[sel])), rel=0.02)
