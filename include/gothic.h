@@ -1,0 +1,139 @@
+/*
+ * gothic.h -- C ABI of the B200-native GOTHIC hot path (Miki & Umemura, arxiv 1610.07279).
+ *
+ * What the library computes: Plummer-softened gravitational accelerations and potentials (eq. 1)
+ * of the currently ACTIVE i-particles of a block time step, approximated by an oct-tree
+ * walk over monopole pseudo j-particles under a multipole acceptance criterion (eq. 2 / eq. 5,
+ * PAPER.md:68-89), plus the tree build (App. A) and block-step bookkeeping that feed it.
+ *
+ * Conventions
+ *   - G = 1.  Positions, masses, outputs are FP32.
+ *   - Unless a parameter says HOST, every array pointer is a DEVICE pointer owned by the caller; the library
+ *     never frees or reallocates caller memory.  `stream` is a cudaStream_t passed as void* (NULL = default
+ *     stream).  Calls enqueue work on `stream` and return without synchronising unless stated.
+ *   - "sorted order" s: position in the space-filling-curve order produced by gothic_build_tree;
+ *     perm[s] = original index of the particle at sorted position s.
+ *   - Return value: 0 = GOTHIC_OK, negative = error.  Nothing throws or aborts.  On error outputs are
+ *     unspecified.  An asynchronous capacity overflow (node pool, traversal stack) sets a device flag that
+ *     gothic_get_tree_view / gothic_check report as GOTHIC_ERR_CAPACITY.
+ *   - One context per stream; a context is not thread-safe.
+ *   - There is no CPU fallback: without a CUDA device every compute call returns GOTHIC_ERR_CUDA.
+ */
+#ifndef GOTHIC_B200_H
+#define GOTHIC_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gothic_ctx gothic_ctx; /* opaque: owns keys, permutation, sorted positions, nodes, scratch */
+
+enum {
+    GOTHIC_OK = 0,
+    GOTHIC_ERR_ARG = -1,           /* bad argument (NULL, n = 0, n > n_max, eps <= 0, ...) */
+    GOTHIC_ERR_STATE = -2,         /* walk / update before a successful build */
+    GOTHIC_ERR_CAPACITY = -3,      /* node pool or traversal stack overflow */
+    GOTHIC_ERR_CUDA = -4,          /* CUDA runtime error (see gothic_last_cuda_error) */
+    GOTHIC_ERR_UNIMPLEMENTED = -5
+};
+
+enum { GOTHIC_KEY_PEANO_HILBERT = 0, GOTHIC_KEY_MORTON = 1 };   /* PAPER.md:54 / PAPER.md:564 */
+enum { GOTHIC_MAC_ACCELERATION = 0, GOTHIC_MAC_OPENING_ANGLE = 1 }; /* eq. 5 PAPER.md:85-89 / eq. 2 */
+
+/* Allocates a context for up to n_max particles.
+ *   node_max      node pool capacity; 0 -> 2*n_max (+64).  Must be < 2^28.
+ *   group_size    G: number of consecutive sorted indices that share one traversal (PAPER.md:103-109,
+ *                 "T_sub"; R3): 8, 16 or 32; 0 -> 32.  With G < 32 the spare lanes of the warp split
+ *                 each i-particle's interaction list (ij-parallelisation, S = 32/G).
+ *   scratch_bytes extra scratch for the traversal stacks; 0 -> automatic.
+ * Synchronous (allocates device memory). */
+int gothic_create(gothic_ctx **out, uint32_t n_max, uint32_t node_max, int group_size, size_t scratch_bytes);
+void gothic_destroy(gothic_ctx *ctx);
+const char *gothic_strerror(int code);       /* static strings */
+const char *gothic_last_cuda_error(gothic_ctx *ctx); /* text of the last CUDA error seen by this context */
+
+/* Tree build, PAPER.md:52-62 + App. A (steps B1-B6 of DESIGN.md):
+ * root box -> 63-bit Peano-Hilbert (Listing 1) or Morton (Listing 3) keys -> stable radix sort of (key, index)
+ * -> positions gathered into sorted order -> canonical oct-tree (breadth-first node ids, children contiguous)
+ * -> pseudo j-particle moments m_J, r_J, b_J.
+ *   pos_m   float4[n] (x, y, z, m), ORIGINAL order, device.
+ *   n_leaf  a cell with more than n_leaf particles is subdivided (1..64; 0 -> 16).
+ * Synchronises `stream` once (reads back the node count and per-level offsets). */
+int gothic_build_tree(gothic_ctx *ctx, const float *pos_m, uint32_t n, int key_kind, int n_leaf, void *stream);
+
+/* Pseudo j-particle moments only, on the existing topology (the paper recomputes them every step).
+ *   pos_m_sorted  float4[n] in SORTED order, device; NULL -> keep the positions stored at build time.
+ * Asynchronous. */
+int gothic_update_moments(gothic_ctx *ctx, const float *pos_m_sorted, void *stream);
+
+/* Gravity walk for the active i-particles, PAPER.md:95-132 (steps W1-W6 of DESIGN.md).
+ * All index spaces are SORTED order.
+ *   active        ascending sorted indices of the active particles, device; NULL -> all n particles.
+ *   n_active      number of entries of `active` (ignored if active == NULL).
+ *   n_active_dev  optional device uint32 that overrides n_active (lets set_timesteps feed the walk
+ *                 without a host round trip); NULL -> use n_active.
+ *   eps           Plummer softening length, > 0.
+ *   mac_kind      GOTHIC_MAC_ACCELERATION: accept J iff d >= (m_J b_J^2 / (mac_param |a_old|))^(1/4)  (eq. 5)
+ *                 GOTHIC_MAC_OPENING_ANGLE: accept J iff b_J / d <= mac_param                         (eq. 2)
+ *                 d measured from the surface of the group's enclosing ball (eq. 6-7).
+ *   aold          float[n] |a_old| per particle, sorted order; required iff mac_kind == ACCELERATION.
+ *   acc_pot       float4[n] sorted order; ONLY active entries are written: (ax, ay, az, Phi).
+ *   amag_out      optional float[n]: |a| of the new acceleration for active entries (may alias aold).
+ *   n_interactions optional device counter, incremented by sum over groups (#members x list length)
+ *                 (counted in a separate run; pass NULL in timed runs).
+ * Asynchronous. */
+int gothic_walk_tree(gothic_ctx *ctx, const uint32_t *active, uint32_t n_active, const uint32_t *n_active_dev,
+                     float eps, int mac_kind, float mac_param, const float *aold,
+                     float *acc_pot, float *amag_out, unsigned long long *n_interactions, void *stream);
+
+/* Block time steps (criterion from BASELINE.json configs[2], R6):
+ * dt_i = eta sqrt(eps / |a_i|) floored to a power of two; level 0 = finest level present, clamped to
+ * max_levels - 1; a particle is active at `substep` (1-based within the cycle) iff level <= ctz(substep).
+ *   acc_pot       float4[n] accelerations, device; NULL -> keep `level` as is and only emit the active list.
+ *   level         uint8[n] in/out.
+ *   active        uint32[n] out: ascending indices of the active particles.
+ *   n_active_dev  uint32 out (device).
+ *   emin_nlev_dev int32[2] out (device): {exponent of the finest dt, number of levels}; written only when
+ *                 acc_pot != NULL.  May be NULL.
+ * Asynchronous. */
+int gothic_set_timesteps(gothic_ctx *ctx, const float *acc_pot, uint32_t n, float eps, float eta, int max_levels,
+                         uint32_t substep, uint8_t *level, uint32_t *active, uint32_t *n_active_dev,
+                         int32_t *emin_nlev_dev, void *stream);
+
+/* Read-only device views for parity tests; valid until the next build.  Synchronises `stream`. */
+typedef struct {
+    uint32_t n, n_nodes, n_levels_tree, group_size;
+    float box[4];                 /* xmin, ymin, zmin, side */
+    const uint64_t *key;          /* [n] sorted keys */
+    const uint32_t *perm;         /* [n] */
+    const float *pos_m_sorted;    /* float4[n] */
+    const uint32_t *node_head, *node_num, *node_child; /* [n_nodes]; child = 0xFFFFFFFF for a leaf */
+    const uint8_t *node_level, *node_nchild;           /* [n_nodes] */
+    const uint32_t *level_ofs;    /* [23] device: id of the first node of each level */
+    const float *node_com;        /* float4[n_nodes]: r_J, m_J */
+    const float *node_b;          /* [n_nodes]: b_J */
+} gothic_tree_view;
+int gothic_get_tree_view(gothic_ctx *ctx, gothic_tree_view *out, void *stream);
+
+/* Synchronises `stream` and returns GOTHIC_ERR_CAPACITY / GOTHIC_ERR_CUDA if an asynchronous error was
+ * flagged since the last check, else GOTHIC_OK. */
+int gothic_check(gothic_ctx *ctx, void *stream);
+
+/* End-to-end convenience with HOST buffers (bench.py "e2e"): H2D copy of pos_m (and aold), build, one walk of
+ * all particles, D2H copy of acc_pot in SORTED order and of perm.  Synchronises.
+ *   pos_m_host float4[n] HOST; aold_host float[n] HOST in ORIGINAL order (NULL allowed for opening-angle MAC);
+ *   acc_pot_host float4[n] HOST out (sorted order); perm_host uint32[n] HOST out (may be NULL). */
+int gothic_gravity_host(gothic_ctx *ctx, const float *pos_m_host, uint32_t n, int key_kind, int n_leaf,
+                        float eps, int mac_kind, float mac_param, const float *aold_host,
+                        float *acc_pot_host, uint32_t *perm_host, void *stream);
+
+/* Number of kernels this library has launched through this context (bench.py "gpu_launches"). */
+unsigned long long gothic_launch_count(gothic_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GOTHIC_B200_H */

@@ -43,6 +43,8 @@ def lib():
         L.oracle_build_tree.argtypes = [_u64p, C.c_uint32, C.c_int, C.c_uint32, _u32p, _u32p, _u32p, _u8p, _u8p, _u32p]
         L.oracle_moments.restype = None
         L.oracle_moments.argtypes = [_f32p, C.c_uint32, _u32p, _u32p, _f32p, _f32p]
+        L.oracle_radius.restype = None
+        L.oracle_radius.argtypes = [_f32p, C.c_uint32, _u32p, _u32p, _f32p, _f32p]
         L.oracle_levels.restype = None
         L.oracle_levels.argtypes = [_f32p, C.c_uint32, C.c_float, C.c_int, _u8p, _i32p]
         L.oracle_active.restype = C.c_uint32
@@ -150,6 +152,15 @@ def moments(pos_sorted, head, num) -> tuple[np.ndarray, np.ndarray]:
     b = np.zeros(m, np.float32)
     lib().oracle_moments(pos_sorted, m, np.ascontiguousarray(head, np.uint32), np.ascontiguousarray(num, np.uint32), com, b)
     return com, b
+
+
+def radius(pos_sorted, head, num, com) -> np.ndarray:
+    """b_J about the given stored centres (second half of O5)."""
+    m = head.shape[0]
+    b = np.zeros(m, np.float32)
+    lib().oracle_radius(_pos(pos_sorted), m, np.ascontiguousarray(head, np.uint32), np.ascontiguousarray(num, np.uint32),
+                        np.ascontiguousarray(com, np.float32), b)
+    return b
 
 
 def build_tree(pos_m, key_kind: int = 0, n_leaf: int = 16, node_cap: int | None = None) -> Tree:

@@ -260,6 +260,23 @@ void oracle_moments(const float *pos_sorted, uint32_t n_nodes, const uint32_t *h
     }
 }
 
+/* O5, second half only: b_J = max |r_j - r_J| about a GIVEN stored centre com4 (stage-wise parity: the radius a
+ * CUDA build reports is checked against the definition applied to the centre that same build stored). */
+void oracle_radius(const float *pos_sorted, uint32_t n_nodes, const uint32_t *head, const uint32_t *num,
+                   const float *com4, float *b)
+{
+#pragma omp parallel for schedule(dynamic, 256)
+    for (int64_t J = 0; J < (int64_t)n_nodes; J++) {
+        double b2 = 0.0;
+        for (uint32_t j = head[J]; j < head[J] + num[J]; j++) {
+            const float *p = pos_sorted + 4 * (size_t)j;
+            const double dx = (double)p[0] - com4[4 * J], dy = (double)p[1] - com4[4 * J + 1], dz = (double)p[2] - com4[4 * J + 2];
+            b2 = std::max(b2, dx * dx + dy * dy + dz * dz);
+        }
+        b[J] = (float)std::sqrt(b2);
+    }
+}
+
 /* O6 (reading R6; criterion from BASELINE.json configs[2]): dt_i = eta sqrt(eps/|a_i|) floored to a power
  * of two.  q = dt^4 = c / |a|^2 with c = (float)(eta^4 eps^2) formed by the caller; exponent of dt =
  * floor(ilogb(q) / 4).  Levels count up from the finest present, clamped to max_levels - 1. */

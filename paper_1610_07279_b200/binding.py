@@ -1,0 +1,196 @@
+"""Thin ctypes binding over the C ABI in include/gothic.h: argument marshalling only.
+
+Every function takes torch CUDA tensors (device memory + current stream are PyTorch's job, nothing else)
+and passes raw pointers to libgothic_b200.so.  There is no CPU fallback: if the library is missing or a
+call fails, a GothicError is raised."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libgothic_b200.so")
+
+KEY_PEANO_HILBERT, KEY_MORTON = 0, 1
+MAC_ACCELERATION, MAC_OPENING_ANGLE = 0, 1
+
+EXPORTS = [
+    "gothic_create", "gothic_destroy", "gothic_strerror", "gothic_last_cuda_error", "gothic_build_tree",
+    "gothic_update_moments", "gothic_walk_tree", "gothic_set_timesteps", "gothic_get_tree_view", "gothic_check",
+    "gothic_gravity_host", "gothic_launch_count",
+]
+
+
+class GothicError(RuntimeError):
+    pass
+
+
+class TreeViewStruct(C.Structure):
+    _fields_ = [("n", C.c_uint32), ("n_nodes", C.c_uint32), ("n_levels_tree", C.c_uint32), ("group_size", C.c_uint32),
+                ("box", C.c_float * 4),
+                ("key", C.c_void_p), ("perm", C.c_void_p), ("pos_m_sorted", C.c_void_p),
+                ("node_head", C.c_void_p), ("node_num", C.c_void_p), ("node_child", C.c_void_p),
+                ("node_level", C.c_void_p), ("node_nchild", C.c_void_p), ("level_ofs", C.c_void_p),
+                ("node_com", C.c_void_p), ("node_b", C.c_void_p)]
+
+
+_lib = None
+
+
+def load_library():
+    """Loads libgothic_b200.so (built in-tree by paper_1610_07279_b200.build).  Fails loudly if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise GothicError(f"{LIB_PATH} not found: run `python -m paper_1610_07279_b200.build` (no CPU fallback exists)")
+    L = C.CDLL(LIB_PATH)
+    vp, u32, i32, f32 = C.c_void_p, C.c_uint32, C.c_int, C.c_float
+    L.gothic_create.restype = i32
+    L.gothic_create.argtypes = [C.POINTER(vp), u32, u32, i32, C.c_size_t]
+    L.gothic_destroy.restype = None
+    L.gothic_destroy.argtypes = [vp]
+    L.gothic_strerror.restype = C.c_char_p
+    L.gothic_strerror.argtypes = [i32]
+    L.gothic_last_cuda_error.restype = C.c_char_p
+    L.gothic_last_cuda_error.argtypes = [vp]
+    L.gothic_build_tree.restype = i32
+    L.gothic_build_tree.argtypes = [vp, vp, u32, i32, i32, vp]
+    L.gothic_update_moments.restype = i32
+    L.gothic_update_moments.argtypes = [vp, vp, vp]
+    L.gothic_walk_tree.restype = i32
+    L.gothic_walk_tree.argtypes = [vp, vp, u32, vp, f32, i32, f32, vp, vp, vp, vp, vp]
+    L.gothic_set_timesteps.restype = i32
+    L.gothic_set_timesteps.argtypes = [vp, vp, u32, f32, f32, i32, u32, vp, vp, vp, vp, vp]
+    L.gothic_get_tree_view.restype = i32
+    L.gothic_get_tree_view.argtypes = [vp, C.POINTER(TreeViewStruct), vp]
+    L.gothic_check.restype = i32
+    L.gothic_check.argtypes = [vp, vp]
+    L.gothic_gravity_host.restype = i32
+    L.gothic_gravity_host.argtypes = [vp, vp, u32, i32, i32, f32, i32, f32, vp, vp, vp, vp]
+    L.gothic_launch_count.restype = C.c_ulonglong
+    L.gothic_launch_count.argtypes = [vp]
+    _lib = L
+    return L
+
+
+def _ptr(t, dtype=None):
+    if t is None:
+        return None
+    if not t.is_cuda or not t.is_contiguous():
+        raise GothicError("expected a contiguous CUDA tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise GothicError(f"expected dtype {dtype}, got {t.dtype}")
+    return C.c_void_p(t.data_ptr())
+
+
+def _stream():
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+class _DevView:
+    """Wraps a raw device pointer so that torch can alias it (__cuda_array_interface__)."""
+
+    def __init__(self, ptr: int, count: int, typestr: str):
+        self.__cuda_array_interface__ = {"shape": (count,), "typestr": typestr, "data": (int(ptr), False), "version": 2}
+
+
+_TYPESTR = {torch.int64: "<i8", torch.int32: "<i4", torch.uint8: "|u1", torch.float32: "<f4"}
+
+
+def _from_ptr(ptr: int, count: int, dtype: torch.dtype, device) -> torch.Tensor:
+    """Copies `count` elements of device memory at `ptr` into a new tensor (parity tests only)."""
+    if count == 0 or not ptr:
+        return torch.empty(count, dtype=dtype, device=device)
+    return torch.as_tensor(_DevView(ptr, count, _TYPESTR[dtype]), device=device).clone()
+
+
+class Gothic:
+    """One context = one tree + scratch on the current CUDA device.  Method names follow the C ABI."""
+
+    def __init__(self, n_max: int, node_max: int = 0, group_size: int = 32, scratch_bytes: int = 0):
+        self._L = load_library()
+        if not torch.cuda.is_available():
+            raise GothicError("no CUDA device: the GOTHIC hot path has no CPU fallback")
+        self._ctx = C.c_void_p()
+        self._chk(self._L.gothic_create(C.byref(self._ctx), n_max, node_max, group_size, scratch_bytes), create=True)
+        self.n_max, self.group_size = n_max, group_size or 32
+        self.device = torch.device("cuda", torch.cuda.current_device())
+
+    def _chk(self, rc: int, create: bool = False):
+        if rc != 0:
+            msg = self._L.gothic_strerror(rc).decode()
+            if rc == -4 and not create and self._ctx:
+                msg += ": " + self._L.gothic_last_cuda_error(self._ctx).decode()
+            raise GothicError(f"gothic error {rc}: {msg}")
+
+    def close(self):
+        if getattr(self, "_ctx", None):
+            self._L.gothic_destroy(self._ctx)
+            self._ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- the C-ABI calls -----------------------------------------------------------------------------------
+    def build_tree(self, pos_m: torch.Tensor, key_kind: int = KEY_PEANO_HILBERT, n_leaf: int = 16):
+        self._chk(self._L.gothic_build_tree(self._ctx, _ptr(pos_m, torch.float32), pos_m.shape[0], key_kind, n_leaf, _stream()))
+
+    def update_moments(self, pos_m_sorted: torch.Tensor | None = None):
+        self._chk(self._L.gothic_update_moments(self._ctx, _ptr(pos_m_sorted, torch.float32), _stream()))
+
+    def walk_tree(self, acc_pot: torch.Tensor, *, eps: float, mac_kind: int, mac_param: float, aold: torch.Tensor | None = None,
+                  active: torch.Tensor | None = None, n_active: int | None = None, n_active_dev: torch.Tensor | None = None,
+                  amag_out: torch.Tensor | None = None, n_interactions: torch.Tensor | None = None):
+        na = 0
+        if active is not None:
+            na = int(active.shape[0] if n_active is None else n_active)
+        self._chk(self._L.gothic_walk_tree(self._ctx, _ptr(active, torch.int32) if active is not None else None, na,
+                                           _ptr(n_active_dev, torch.int32), float(eps), mac_kind, float(mac_param),
+                                           _ptr(aold, torch.float32), _ptr(acc_pot, torch.float32), _ptr(amag_out, torch.float32),
+                                           _ptr(n_interactions, torch.int64), _stream()))
+
+    def set_timesteps(self, level: torch.Tensor, *, acc_pot: torch.Tensor | None, eps: float, eta: float = 0.5, max_levels: int = 8,
+                      substep: int = 1, active: torch.Tensor | None = None, n_active_dev: torch.Tensor | None = None,
+                      emin_nlev_dev: torch.Tensor | None = None):
+        self._chk(self._L.gothic_set_timesteps(self._ctx, _ptr(acc_pot, torch.float32), level.shape[0], float(eps), float(eta),
+                                               max_levels, substep, _ptr(level, torch.uint8), _ptr(active, torch.int32),
+                                               _ptr(n_active_dev, torch.int32), _ptr(emin_nlev_dev, torch.int32), _stream()))
+
+    def check(self):
+        self._chk(self._L.gothic_check(self._ctx, _stream()))
+
+    def launch_count(self) -> int:
+        return int(self._L.gothic_launch_count(self._ctx))
+
+    def get_tree_view(self) -> dict:
+        """Copies of the tree arrays as torch tensors (parity tests; synchronises)."""
+        v = TreeViewStruct()
+        self._chk(self._L.gothic_get_tree_view(self._ctx, C.byref(v), _stream()))
+        torch.cuda.current_stream().synchronize()
+        d, n, m = self.device, v.n, v.n_nodes
+        return dict(
+            n=n, n_nodes=m, n_levels_tree=v.n_levels_tree, group_size=v.group_size, box=[float(x) for x in v.box],
+            key=_from_ptr(v.key, n, torch.int64, d), perm=_from_ptr(v.perm, n, torch.int32, d),
+            pos_m_sorted=_from_ptr(v.pos_m_sorted, 4 * n, torch.float32, d).view(n, 4),
+            node_head=_from_ptr(v.node_head, m, torch.int32, d), node_num=_from_ptr(v.node_num, m, torch.int32, d),
+            node_child=_from_ptr(v.node_child, m, torch.int32, d), node_level=_from_ptr(v.node_level, m, torch.uint8, d),
+            node_nchild=_from_ptr(v.node_nchild, m, torch.uint8, d), level_ofs=_from_ptr(v.level_ofs, 23, torch.int32, d),
+            node_com=_from_ptr(v.node_com, 4 * m, torch.float32, d).view(m, 4), node_b=_from_ptr(v.node_b, m, torch.float32, d),
+        )
+
+    def gravity_host(self, pos_m_host: torch.Tensor, acc_pot_host: torch.Tensor, *, eps: float, mac_kind: int, mac_param: float,
+                     aold_host: torch.Tensor | None = None, perm_host: torch.Tensor | None = None,
+                     key_kind: int = KEY_PEANO_HILBERT, n_leaf: int = 16):
+        """End to end with HOST (pinned) buffers: H2D, build, all-active walk, D2H."""
+        for t in (pos_m_host, acc_pot_host, aold_host, perm_host):
+            if t is not None and (t.is_cuda or not t.is_contiguous()):
+                raise GothicError("gravity_host expects contiguous host tensors")
+        hp = lambda t: None if t is None else C.c_void_p(t.data_ptr())
+        self._chk(self._L.gothic_gravity_host(self._ctx, hp(pos_m_host), pos_m_host.shape[0], key_kind, n_leaf, float(eps), mac_kind,
+                                              float(mac_param), hp(aold_host), hp(acc_pot_host), hp(perm_host), _stream()))

@@ -1,0 +1,224 @@
+// B5: canonical oct-tree (node ranges + links) from the sorted keys, all levels at once.
+//
+// PAPER.md:58 builds the tree breadth-first, one level per grid-wide barrier (Xiao & Feng lock-free barrier,
+// PAPER.md:60).  On B200 that chain of <= 21 dependent grid syncs is replaced by a formulation in which every
+// level is independent, so the whole topology comes out of two streaming passes over the keys:
+//
+//   delta(p)  = number of leading octal digits shared by key[p-1] and key[p]   (delta(0) = delta(n) = -1)
+//   D(p)      = deepest level at which the run of equal-prefix keys containing p holds more than n_leaf
+//               particles = max over windows [i, i+n_leaf] containing p of shared_digits(key[i], key[i+n_leaf])
+//   p STARTS a node at every level L in [delta(p)+1, min(D(p)+1, 21)]
+//   p ENDS   a node at every level L in [delta(p+1)+1, min(D(p)+1, 21)]
+//
+// (a level-L run is a node iff its parent run has more than n_leaf particles, and run sizes shrink monotonically
+// with depth).  The k-th start and the k-th end of a level belong to the same node; node id = level offset +
+// rank, which is exactly breadth-first order with ascending head inside a level, so children are contiguous.
+// Pass 1 counts start/end events per (block, level); a small scan turns them into offsets; pass 2 emits.
+#include "gothic_ctx.cuh"
+
+namespace {
+
+constexpr int TPB = 256;
+constexpr int NW = TPB / 32;
+
+struct Events { int s_lo, s_hi, e_lo, e_hi; };
+
+__device__ __forceinline__ Events node_events(const uint64_t *sk, int tid, uint32_t p, uint32_t n, int H)
+{
+    Events ev = {1, 0, 1, 0};
+    if (p < n) {
+        const uint64_t kp = sk[H + tid];
+        const int dprev = p == 0 ? -1 : shared_digits(sk[H + tid - 1], kp);
+        const int dnext = p == n - 1 ? -1 : shared_digits(kp, sk[H + tid + 1]);
+        int D = -1;
+        for (int w = 0; w <= H; w++) {
+            const long long i = (long long)p - H + w;
+            if (i >= 0 && i + H < (long long)n) D = max(D, shared_digits(sk[tid + w], sk[tid + w + H]));
+        }
+        const int top = min(D + 1, GOTHIC_NLEV);
+        ev.s_lo = dprev + 1; ev.s_hi = top; ev.e_lo = dnext + 1; ev.e_hi = top;
+    }
+    return ev;
+}
+
+__device__ __forceinline__ void load_keys(uint64_t *sk, const uint64_t *__restrict__ key, uint32_t n, int H)
+{
+    const long long base = (long long)blockIdx.x * TPB - H;
+    for (int t = threadIdx.x; t < TPB + 2 * H; t += TPB) {
+        const long long g = base + t;
+        sk[t] = (g >= 0 && g < (long long)n) ? __ldg(key + g) : 0ull;
+    }
+    __syncthreads();
+}
+
+// blk_cnt layout: [kind(0 = start, 1 = end)][level][nblk]
+__global__ void __launch_bounds__(TPB) k_count_events(const uint64_t *__restrict__ key, uint32_t n, int H,
+                                                       uint32_t *__restrict__ blk_cnt, uint32_t nblk)
+{
+    __shared__ uint64_t sk[TPB + 2 * GOTHIC_MAX_NLEAF];
+    __shared__ uint32_t tot[2][GOTHIC_NLEVP1];
+    if (threadIdx.x < 2 * GOTHIC_NLEVP1) (&tot[0][0])[threadIdx.x] = 0;
+    load_keys(sk, key, n, H);
+    const Events ev = node_events(sk, threadIdx.x, blockIdx.x * TPB + threadIdx.x, n, H);
+#pragma unroll
+    for (int L = 0; L < GOTHIC_NLEVP1; L++) {
+        const uint32_t bs = __ballot_sync(0xffffffffu, ev.s_lo <= L && L <= ev.s_hi);
+        const uint32_t be = __ballot_sync(0xffffffffu, ev.e_lo <= L && L <= ev.e_hi);
+        if (lane_id() == 0) {
+            if (bs) atomicAdd(&tot[0][L], __popc(bs));
+            if (be) atomicAdd(&tot[1][L], __popc(be));
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x < 2 * GOTHIC_NLEVP1)
+        blk_cnt[(size_t)threadIdx.x * nblk + blockIdx.x] = (&tot[0][0])[threadIdx.x];
+}
+
+// One block per (kind, level): exclusive scan over blocks in place; totals of the start rows -> level_cnt.
+__global__ void __launch_bounds__(TPB) k_scan_blocks(uint32_t *__restrict__ blk_cnt, uint32_t nblk, uint32_t *__restrict__ level_cnt)
+{
+    __shared__ uint32_t wsum[NW];
+    __shared__ uint32_t carry_s;
+    uint32_t *row = blk_cnt + (size_t)blockIdx.x * nblk;
+    if (threadIdx.x == 0) carry_s = 0;
+    __syncthreads();
+    for (uint32_t b0 = 0; b0 < nblk; b0 += TPB) {
+        const uint32_t i = b0 + threadIdx.x;
+        const uint32_t v = i < nblk ? row[i] : 0u;
+        uint32_t x = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
+            if ((int)lane_id() >= o) x += y;
+        }
+        if (lane_id() == 31) wsum[threadIdx.x >> 5] = x;
+        __syncthreads();
+        uint32_t wpre = 0, total = 0;
+#pragma unroll
+        for (int w = 0; w < NW; w++) {
+            const uint32_t s = wsum[w];
+            if (w < (int)(threadIdx.x >> 5)) wpre += s;
+            total += s;
+        }
+        const uint32_t carry = carry_s;
+        if (i < nblk) row[i] = carry + wpre + x - v;
+        __syncthreads();
+        if (threadIdx.x == 0) carry_s = carry + total;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0 && blockIdx.x < GOTHIC_NLEVP1) level_cnt[blockIdx.x] = carry_s;
+}
+
+// level offsets, node count, capacity check.  flags[0] = overflow, flags[2] = n_nodes
+__global__ void k_level_offsets(const uint32_t *level_cnt, uint32_t *level_ofs, uint32_t *flags, uint32_t node_max)
+{
+    unsigned long long acc = 0;
+    for (int L = 0; L < GOTHIC_NLEVP1; L++) {
+        level_ofs[L] = (uint32_t)min(acc, 0xFFFFFFFFull);
+        acc += level_cnt[L];
+    }
+    level_ofs[GOTHIC_NLEVP1] = (uint32_t)min(acc, 0xFFFFFFFFull);
+    flags[2] = (uint32_t)min(acc, 0xFFFFFFFFull);
+    if (acc > node_max) flags[0] = 1u;
+}
+
+__global__ void __launch_bounds__(TPB) k_emit_nodes(const uint64_t *__restrict__ key, uint32_t n, int H,
+                                                     const uint32_t *__restrict__ blk_cnt, uint32_t nblk,
+                                                     const uint32_t *__restrict__ level_ofs, const uint32_t *__restrict__ flags,
+                                                     uint32_t *__restrict__ node_head, uint8_t *__restrict__ node_level,
+                                                     uint32_t *__restrict__ node_child, uint32_t *__restrict__ node_end,
+                                                     uint32_t *__restrict__ node_last)
+{
+    __shared__ uint64_t sk[TPB + 2 * GOTHIC_MAX_NLEAF];
+    __shared__ uint32_t wcnt[2][GOTHIC_NLEVP1][NW];   // per-warp counts -> exclusive prefix + block base + level offset
+    if (flags[0]) return;
+    load_keys(sk, key, n, H);
+    const uint32_t p = blockIdx.x * TPB + threadIdx.x;
+    const Events ev = node_events(sk, threadIdx.x, p, n, H);
+    const int warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int L = 0; L < GOTHIC_NLEVP1; L++) {
+        const uint32_t bs = __ballot_sync(0xffffffffu, ev.s_lo <= L && L <= ev.s_hi);
+        const uint32_t be = __ballot_sync(0xffffffffu, ev.e_lo <= L && L <= ev.e_hi);
+        if (lane_id() == 0) { wcnt[0][L][warp] = __popc(bs); wcnt[1][L][warp] = __popc(be); }
+    }
+    __syncthreads();
+    if (threadIdx.x < 2 * GOTHIC_NLEVP1) {
+        const int kind = threadIdx.x / GOTHIC_NLEVP1, L = threadIdx.x % GOTHIC_NLEVP1;
+        uint32_t run = level_ofs[L] + blk_cnt[(size_t)threadIdx.x * nblk + blockIdx.x];
+#pragma unroll
+        for (int w = 0; w < NW; w++) { const uint32_t c = wcnt[kind][L][w]; wcnt[kind][L][w] = run; run += c; }
+    }
+    __syncthreads();
+    const uint32_t lt = (1u << lane_id()) - 1u;
+    uint32_t sid_below = GOTHIC_LEAF, eid_below = GOTHIC_LEAF;   // ids of this thread's events one level deeper
+#pragma unroll
+    for (int L = GOTHIC_NLEV; L >= 0; L--) {
+        const bool fs = ev.s_lo <= L && L <= ev.s_hi, fe = ev.e_lo <= L && L <= ev.e_hi;
+        const uint32_t bs = __ballot_sync(0xffffffffu, fs);
+        const uint32_t be = __ballot_sync(0xffffffffu, fe);
+        if (fs) {
+            const uint32_t id = wcnt[0][L][warp] + __popc(bs & lt);
+            node_head[id] = p;
+            node_level[id] = (uint8_t)L;
+            node_child[id] = (L + 1 <= ev.s_hi) ? sid_below : GOTHIC_LEAF;
+            sid_below = id;
+        }
+        if (fe) {
+            const uint32_t id = wcnt[1][L][warp] + __popc(be & lt);
+            node_end[id] = p + 1;
+            node_last[id] = (L + 1 <= ev.e_hi) ? eid_below : GOTHIC_LEAF;
+            eid_below = id;
+        }
+    }
+}
+
+__global__ void __launch_bounds__(TPB) k_finish_nodes(uint32_t n_nodes, const uint32_t *__restrict__ node_head,
+                                                       const uint32_t *__restrict__ node_end, const uint32_t *__restrict__ node_child,
+                                                       const uint32_t *__restrict__ node_last, uint32_t *__restrict__ node_num,
+                                                       uint8_t *__restrict__ node_nchild, uint32_t *__restrict__ node_parent)
+{
+    const uint32_t J = blockIdx.x * TPB + threadIdx.x;
+    if (J >= n_nodes) return;
+    node_num[J] = node_end[J] - node_head[J];
+    const uint32_t c = node_child[J];
+    uint32_t nc = 0;
+    if (c != GOTHIC_LEAF) {
+        nc = node_last[J] - c + 1u;
+        for (uint32_t k = 0; k < nc; k++) node_parent[c + k] = J;
+    }
+    node_nchild[J] = (uint8_t)nc;
+    if (J == 0) node_parent[0] = GOTHIC_LEAF;
+}
+
+} // namespace
+
+int gothic_stage_nodes(gothic_ctx *c, uint32_t n, int n_leaf, cudaStream_t s)
+{
+    const uint32_t nblk = (n + TPB - 1) / TPB;
+    const uint64_t *key = c->key[c->cur];
+    GOTHIC_CUDA_OK(c, cudaMemsetAsync(c->flags, 0, 4 * sizeof(uint32_t), s));
+    k_count_events<<<nblk, TPB, 0, s>>>(key, n, n_leaf, c->blk_cnt, nblk);
+    GOTHIC_LAUNCH_OK(c);
+    k_scan_blocks<<<2 * GOTHIC_NLEVP1, TPB, 0, s>>>(c->blk_cnt, nblk, c->level_cnt);
+    GOTHIC_LAUNCH_OK(c);
+    k_level_offsets<<<1, 1, 0, s>>>(c->level_cnt, c->level_ofs, c->flags, c->node_max);
+    GOTHIC_LAUNCH_OK(c);
+    k_emit_nodes<<<nblk, TPB, 0, s>>>(key, n, n_leaf, c->blk_cnt, nblk, c->level_ofs, c->flags, c->node_head, c->node_level,
+                                      c->node_child, c->node_end, c->node_last);
+    GOTHIC_LAUNCH_OK(c);
+    // the one host read of the build: node count + level offsets (sizes the remaining launches)
+    uint32_t h_flags[4];
+    GOTHIC_CUDA_OK(c, cudaMemcpyAsync(c->h_level_ofs, c->level_ofs, (GOTHIC_NLEVP1 + 1) * sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
+    GOTHIC_CUDA_OK(c, cudaMemcpyAsync(h_flags, c->flags, sizeof(h_flags), cudaMemcpyDeviceToHost, s));
+    GOTHIC_CUDA_OK(c, cudaStreamSynchronize(s));
+    if (h_flags[0]) return GOTHIC_ERR_CAPACITY;
+    c->n_nodes = h_flags[2];
+    c->n_levels_tree = 0;
+    for (int L = 0; L < GOTHIC_NLEVP1; L++)
+        if (c->h_level_ofs[L + 1] > c->h_level_ofs[L]) c->n_levels_tree = L + 1;
+    k_finish_nodes<<<(c->n_nodes + TPB - 1) / TPB, TPB, 0, s>>>(c->n_nodes, c->node_head, c->node_end, c->node_child, c->node_last,
+                                                                c->node_num, c->node_nchild, c->node_parent);
+    GOTHIC_LAUNCH_OK(c);
+    return GOTHIC_OK;
+}

@@ -1,0 +1,257 @@
+// C-ABI entry points of libgothic_b200 (include/gothic.h).  Host logic only: argument checks, buffer
+// ownership, stage sequencing.  Every step of the path runs in the kernels of the other translation units.
+#include "gothic_ctx.cuh"
+#include <new>
+#include <string.h>
+
+namespace {
+
+template <typename T>
+cudaError_t dev_alloc(T **p, size_t count)
+{
+    return cudaMalloc(reinterpret_cast<void **>(p), count * sizeof(T));
+}
+
+void free_all(gothic_ctx *c)
+{
+    void *ptrs[] = {c->key[0], c->key[1], c->idx[0], c->idx[1], c->pos_sorted, c->box, c->bbox_bits,
+                    c->node_head, c->node_num, c->node_child, c->node_parent, c->node_end, c->node_last,
+                    c->node_level, c->node_nchild, c->node_com, c->node_msum, c->node_b, c->node_b2bits, c->node_rec,
+                    c->level_ofs, c->level_cnt, c->blk_cnt, c->flags, c->sort_tmp, c->grp_mask, c->grp_list, c->grp_cnt,
+                    c->stack, c->ts_tmp, c->scan_tmp, c->h2d_pos, c->h2d_aold, c->d_aold_sorted, c->d_acc};
+    for (void *p : ptrs)
+        if (p) cudaFree(p);
+}
+
+__global__ void k_gather_f32(const float *__restrict__ src, const uint32_t *__restrict__ perm, uint32_t n, float *__restrict__ dst)
+{
+    const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s < n) dst[s] = __ldg(src + __ldg(perm + s));
+}
+
+} // namespace
+
+extern "C" {
+
+const char *gothic_strerror(int code)
+{
+    switch (code) {
+    case GOTHIC_OK: return "ok";
+    case GOTHIC_ERR_ARG: return "invalid argument";
+    case GOTHIC_ERR_STATE: return "tree not built";
+    case GOTHIC_ERR_CAPACITY: return "node pool or traversal stack capacity exceeded";
+    case GOTHIC_ERR_CUDA: return "CUDA runtime error";
+    case GOTHIC_ERR_UNIMPLEMENTED: return "not implemented";
+    default: return "unknown error";
+    }
+}
+
+const char *gothic_last_cuda_error(gothic_ctx *ctx)
+{
+    return ctx ? cudaGetErrorString(ctx->last_err) : "no context";
+}
+
+int gothic_create(gothic_ctx **out, uint32_t n_max, uint32_t node_max, int group_size, size_t scratch_bytes)
+{
+    if (!out || n_max == 0 || n_max > (1u << 31)) return GOTHIC_ERR_ARG;
+    if (group_size == 0) group_size = 32;
+    if (group_size != 8 && group_size != 16 && group_size != 32) return GOTHIC_ERR_ARG;
+    if (node_max == 0) {
+        const unsigned long long d = 2ull * n_max + 64ull;
+        node_max = d >= (1ull << 28) ? (1u << 28) - 1u : (uint32_t)d;
+    }
+    if (node_max >= (1u << 28)) return GOTHIC_ERR_ARG;
+    gothic_ctx *c = new (std::nothrow) gothic_ctx;
+    if (!c) return GOTHIC_ERR_ARG;
+    memset(c, 0, sizeof(*c));
+    c->n_max = n_max;
+    c->node_max = node_max;
+    c->group_size = group_size;
+    c->last_err = cudaSuccess;
+    *out = c;
+    cudaError_t e = cudaGetDevice(&c->device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device);
+    if (e != cudaSuccess) { c->last_err = e; delete c; *out = nullptr; return GOTHIC_ERR_CUDA; }
+    gothic_walk_config(c);
+    c->stack_cap = 4096;
+    if (scratch_bytes) {
+        const size_t per = scratch_bytes / ((size_t)c->walk_warps * sizeof(uint32_t));
+        if (per < 512) { delete c; *out = nullptr; return GOTHIC_ERR_ARG; }
+        c->stack_cap = (uint32_t)(per > (1u << 20) ? (1u << 20) : per);
+    }
+    c->nblk_max = (n_max + 255u) / 256u;
+    c->sort_tmp_bytes = gothic_sort_scratch_bytes(n_max);
+    const size_t n_groups = ((size_t)n_max + group_size - 1) / group_size;
+    const size_t n = n_max, m = node_max;
+#define A(expr) if (e == cudaSuccess) e = (expr)
+    A(dev_alloc(&c->key[0], n)); A(dev_alloc(&c->key[1], n));
+    A(dev_alloc(&c->idx[0], n)); A(dev_alloc(&c->idx[1], n));
+    A(dev_alloc(&c->pos_sorted, n));
+    A(dev_alloc(&c->box, 8)); A(dev_alloc(&c->bbox_bits, 8));
+    A(dev_alloc(&c->node_head, m)); A(dev_alloc(&c->node_num, m)); A(dev_alloc(&c->node_child, m));
+    A(dev_alloc(&c->node_parent, m)); A(dev_alloc(&c->node_end, m)); A(dev_alloc(&c->node_last, m));
+    A(dev_alloc(&c->node_level, m)); A(dev_alloc(&c->node_nchild, m));
+    A(dev_alloc(&c->node_com, m)); A(dev_alloc(&c->node_msum, m)); A(dev_alloc(&c->node_b, m));
+    A(dev_alloc(&c->node_b2bits, m)); A(dev_alloc(&c->node_rec, m));
+    A(dev_alloc(&c->level_ofs, GOTHIC_NLEVP1 + 2)); A(dev_alloc(&c->level_cnt, GOTHIC_NLEVP1 + 2));
+    A(dev_alloc(&c->blk_cnt, (size_t)2 * GOTHIC_NLEVP1 * c->nblk_max));
+    A(dev_alloc(&c->flags, 4));
+    A(cudaMalloc(&c->sort_tmp, c->sort_tmp_bytes));
+    A(dev_alloc(&c->grp_mask, n_groups)); A(dev_alloc(&c->grp_list, n_groups)); A(dev_alloc(&c->grp_cnt, 4));
+    A(dev_alloc(&c->stack, (size_t)c->walk_warps * c->stack_cap));
+    A(dev_alloc(&c->ts_tmp, 4)); A(dev_alloc(&c->scan_tmp, (n + 2047) / 2048 + 1));
+    A(cudaMemset(c->flags, 0, 4 * sizeof(uint32_t)));
+#undef A
+    if (e != cudaSuccess) {
+        c->last_err = e;
+        free_all(c);
+        delete c;
+        *out = nullptr;
+        return GOTHIC_ERR_CUDA;
+    }
+    return GOTHIC_OK;
+}
+
+void gothic_destroy(gothic_ctx *ctx)
+{
+    if (!ctx) return;
+    free_all(ctx);
+    delete ctx;
+}
+
+unsigned long long gothic_launch_count(gothic_ctx *ctx) { return ctx ? ctx->launches : 0ull; }
+
+int gothic_build_tree(gothic_ctx *c, const float *pos_m, uint32_t n, int key_kind, int n_leaf, void *stream)
+{
+    if (!c || !pos_m || n == 0 || n > c->n_max) return GOTHIC_ERR_ARG;
+    if (key_kind != GOTHIC_KEY_PEANO_HILBERT && key_kind != GOTHIC_KEY_MORTON) return GOTHIC_ERR_ARG;
+    if (n_leaf == 0) n_leaf = 16;
+    if (n_leaf < 1 || n_leaf > GOTHIC_MAX_NLEAF) return GOTHIC_ERR_ARG;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    const float4 *pos = reinterpret_cast<const float4 *>(pos_m);
+    c->built = false;
+    c->n = n;
+    c->n_leaf = n_leaf;
+    int rc;
+    if ((rc = gothic_stage_keys(c, pos, n, key_kind, s)) != GOTHIC_OK) return rc;
+    if ((rc = gothic_stage_sort(c, n, s)) != GOTHIC_OK) return rc;
+    if ((rc = gothic_stage_gather(c, pos, n, s)) != GOTHIC_OK) return rc;
+    if ((rc = gothic_stage_nodes(c, n, n_leaf, s)) != GOTHIC_OK) return rc;
+    if ((rc = gothic_stage_moments(c, s)) != GOTHIC_OK) return rc;
+    c->built = true;
+    return GOTHIC_OK;
+}
+
+int gothic_update_moments(gothic_ctx *c, const float *pos_m_sorted, void *stream)
+{
+    if (!c) return GOTHIC_ERR_ARG;
+    if (!c->built) return GOTHIC_ERR_STATE;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    if (pos_m_sorted && pos_m_sorted != reinterpret_cast<const float *>(c->pos_sorted))
+        GOTHIC_CUDA_OK(c, cudaMemcpyAsync(c->pos_sorted, pos_m_sorted, (size_t)c->n * sizeof(float4), cudaMemcpyDeviceToDevice, s));
+    return gothic_stage_moments(c, s);
+}
+
+int gothic_walk_tree(gothic_ctx *c, const uint32_t *active, uint32_t n_active, const uint32_t *n_active_dev,
+                     float eps, int mac_kind, float mac_param, const float *aold,
+                     float *acc_pot, float *amag_out, unsigned long long *n_interactions, void *stream)
+{
+    if (!c || !acc_pot || !(eps > 0.0f) || !(mac_param >= 0.0f)) return GOTHIC_ERR_ARG;
+    if (mac_kind != GOTHIC_MAC_ACCELERATION && mac_kind != GOTHIC_MAC_OPENING_ANGLE) return GOTHIC_ERR_ARG;
+    if (mac_kind == GOTHIC_MAC_ACCELERATION && !aold) return GOTHIC_ERR_ARG;
+    if (!c->built) return GOTHIC_ERR_STATE;
+    if (active && !n_active_dev && n_active > c->n) return GOTHIC_ERR_ARG;
+    if (active && !n_active_dev && n_active == 0) return GOTHIC_OK;
+    return gothic_stage_walk(c, active, n_active, n_active_dev, eps, mac_kind, mac_param, aold,
+                             reinterpret_cast<float4 *>(acc_pot), amag_out, n_interactions, static_cast<cudaStream_t>(stream));
+}
+
+int gothic_set_timesteps(gothic_ctx *c, const float *acc_pot, uint32_t n, float eps, float eta, int max_levels,
+                         uint32_t substep, uint8_t *level, uint32_t *active, uint32_t *n_active_dev,
+                         int32_t *emin_nlev_dev, void *stream)
+{
+    if (!c || !level || n == 0 || n > c->n_max) return GOTHIC_ERR_ARG;
+    if (max_levels < 1 || max_levels > 32 || substep == 0) return GOTHIC_ERR_ARG;
+    if ((active == nullptr) != (n_active_dev == nullptr)) return GOTHIC_ERR_ARG;
+    if (acc_pot && (!(eps > 0.0f) || !(eta > 0.0f))) return GOTHIC_ERR_ARG;
+    // c = (float)(eta^4 eps^2), formed once in double then rounded (R6)
+    const double e4 = (double)eta * (double)eta * (double)eta * (double)eta;
+    const float cconst = (float)(e4 * (double)eps * (double)eps);
+    return gothic_stage_timesteps(c, reinterpret_cast<const float4 *>(acc_pot), n, cconst, max_levels, substep, level, active,
+                                  n_active_dev, emin_nlev_dev, static_cast<cudaStream_t>(stream));
+}
+
+int gothic_check(gothic_ctx *c, void *stream)
+{
+    if (!c) return GOTHIC_ERR_ARG;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    uint32_t h[4];
+    GOTHIC_CUDA_OK(c, cudaMemcpyAsync(h, c->flags, sizeof(h), cudaMemcpyDeviceToHost, s));
+    GOTHIC_CUDA_OK(c, cudaStreamSynchronize(s));
+    if (h[0] || h[1]) {
+        const uint32_t zero[2] = {0u, 0u};
+        cudaMemcpyAsync(c->flags, zero, sizeof(zero), cudaMemcpyHostToDevice, s);
+        cudaStreamSynchronize(s);
+        return GOTHIC_ERR_CAPACITY;
+    }
+    return GOTHIC_OK;
+}
+
+int gothic_get_tree_view(gothic_ctx *c, gothic_tree_view *out, void *stream)
+{
+    if (!c || !out) return GOTHIC_ERR_ARG;
+    if (!c->built) return GOTHIC_ERR_STATE;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    float hbox[8];
+    GOTHIC_CUDA_OK(c, cudaMemcpyAsync(hbox, c->box, sizeof(hbox), cudaMemcpyDeviceToHost, s));
+    const int rc = gothic_check(c, stream);
+    if (rc != GOTHIC_OK) return rc;
+    out->n = c->n;
+    out->n_nodes = c->n_nodes;
+    out->n_levels_tree = c->n_levels_tree;
+    out->group_size = (uint32_t)c->group_size;
+    for (int k = 0; k < 4; k++) out->box[k] = hbox[k];
+    out->key = c->key[c->cur];
+    out->perm = c->idx[c->cur];
+    out->pos_m_sorted = reinterpret_cast<const float *>(c->pos_sorted);
+    out->node_head = c->node_head; out->node_num = c->node_num; out->node_child = c->node_child;
+    out->node_level = c->node_level; out->node_nchild = c->node_nchild;
+    out->level_ofs = c->level_ofs;
+    out->node_com = reinterpret_cast<const float *>(c->node_com);
+    out->node_b = c->node_b;
+    return GOTHIC_OK;
+}
+
+int gothic_gravity_host(gothic_ctx *c, const float *pos_m_host, uint32_t n, int key_kind, int n_leaf,
+                        float eps, int mac_kind, float mac_param, const float *aold_host,
+                        float *acc_pot_host, uint32_t *perm_host, void *stream)
+{
+    if (!c || !pos_m_host || !acc_pot_host || n == 0 || n > c->n_max) return GOTHIC_ERR_ARG;
+    if (mac_kind == GOTHIC_MAC_ACCELERATION && !aold_host) return GOTHIC_ERR_ARG;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    if (!c->h2d_pos) {
+        cudaError_t e = dev_alloc(&c->h2d_pos, c->n_max);
+        if (e == cudaSuccess) e = dev_alloc(&c->h2d_aold, c->n_max);
+        if (e == cudaSuccess) e = dev_alloc(&c->d_aold_sorted, c->n_max);
+        if (e == cudaSuccess) e = dev_alloc(&c->d_acc, c->n_max);
+        if (e != cudaSuccess) { c->last_err = e; return GOTHIC_ERR_CUDA; }
+    }
+    GOTHIC_CUDA_OK(c, cudaMemcpyAsync(c->h2d_pos, pos_m_host, (size_t)n * sizeof(float4), cudaMemcpyHostToDevice, s));
+    if (aold_host)
+        GOTHIC_CUDA_OK(c, cudaMemcpyAsync(c->h2d_aold, aold_host, (size_t)n * sizeof(float), cudaMemcpyHostToDevice, s));
+    int rc = gothic_build_tree(c, reinterpret_cast<const float *>(c->h2d_pos), n, key_kind, n_leaf, stream);
+    if (rc != GOTHIC_OK) return rc;
+    if (aold_host) {
+        k_gather_f32<<<(n + 255u) / 256u, 256, 0, s>>>(c->h2d_aold, c->idx[c->cur], n, c->d_aold_sorted);
+        GOTHIC_LAUNCH_OK(c);
+    }
+    rc = gothic_walk_tree(c, nullptr, 0, nullptr, eps, mac_kind, mac_param, aold_host ? c->d_aold_sorted : nullptr,
+                          reinterpret_cast<float *>(c->d_acc), nullptr, nullptr, stream);
+    if (rc != GOTHIC_OK) return rc;
+    GOTHIC_CUDA_OK(c, cudaMemcpyAsync(acc_pot_host, c->d_acc, (size_t)n * sizeof(float4), cudaMemcpyDeviceToHost, s));
+    if (perm_host)
+        GOTHIC_CUDA_OK(c, cudaMemcpyAsync(perm_host, c->idx[c->cur], (size_t)n * sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
+    return gothic_check(c, stream);
+}
+
+} // extern "C"

@@ -1,0 +1,162 @@
+"""-m gpu parity: the gravity walk (W1-W6) through the C ABI vs the CPU oracle.
+
+Stage-wise identical inputs: the oracle's walk is fed the tree, moments and |a_old|
+the CUDA build produced, so every MAC decision is bit-identical on both sides and the interaction counts must be
+EQUAL; accelerations then differ only by fp32 accumulation + rsqrt.approx.  One end-to-end case (oracle uses its own
+moments) is held to BASELINE.json's tolerances with MAC flips allowed."""
+import numpy as np
+import pytest
+import torch
+
+from paper_1610_07279_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL_999, TOL_MAX, TOL_POT_MEDIAN = 1e-4, 1e-2, 1e-4   # BASELINE.json north_star
+
+
+def _oracle_on_gpu_tree(oracle, v, **kw):
+    return oracle.walk(v["pos_m_sorted"], v["node_head"], v["node_num"], v["node_child"], v["node_nchild"],
+                       v["node_com"], v["node_b"], **kw)
+
+
+def _assert_parity(out, ref, rows):
+    from gpu_util import acc_rel_err
+    e = acc_rel_err(out[rows], ref[rows])
+    assert np.percentile(e, 99.9) <= TOL_999, np.percentile(e, 99.9)
+    assert e.max() <= TOL_MAX, e.max()
+    pe = np.abs(out[rows, 3] - ref[rows, 3]) / np.abs(ref[rows, 3])
+    assert np.median(pe) <= TOL_POT_MEDIAN and pe.max() <= 1e-3, (np.median(pe), pe.max())
+
+
+def _bootstrap_aold(g, n, eps):
+    from gpu_util import gpu_walk
+    out, _, am = gpu_walk(g, n, eps=eps, mac_kind=1, mac_param=0.5, amag=True, count=False)
+    assert np.allclose(am, np.linalg.norm(out[:, :3], axis=1), rtol=1e-6)
+    return am
+
+
+@pytest.mark.parametrize("model,n,G,n_leaf", [("plummer", 1 << 13, 32, 16), ("hernquist", 40001, 32, 16),
+                                                ("nfw", 30000, 16, 16), ("m31_like", 30000, 8, 8), ("plummer", 5000, 32, 4)])
+def test_walk_matches_oracle_all_active(oracle, model, n, G, n_leaf):
+    from gpu_util import gpu_build, gpu_walk
+    pos = getattr(W, model)(n, seed=2)
+    eps = 2.0 ** -7
+    g, v = gpu_build(pos, n_leaf=n_leaf, group_size=G)
+    aold = _bootstrap_aold(g, n, eps)
+    for kind, param in ((0, 2.0 ** -9), (0, 2.0 ** -4), (1, 0.6)):
+        out, cnt, _ = gpu_walk(g, n, eps=eps, mac_kind=kind, mac_param=param, aold=aold)
+        ref, c = _oracle_on_gpu_tree(oracle, v, eps=eps, mac_kind=kind, mac_param=param, aold=aold, group_size=G)
+        assert cnt == c["interactions"]
+        _assert_parity(out, ref, np.arange(n))
+    g.close()
+
+
+@pytest.mark.parametrize("frac,G", [(0.5, 32), (0.1, 32), (0.01, 32), (0.003, 32), (0.1, 16), (0.02, 8)])
+def test_walk_sparse_active_sets(oracle, frac, G):
+    """BASELINE.json configs[4]-style random active subsets: ij-parallel lanes (S > 1) and untouched inactive rows."""
+    from gpu_util import gpu_build, gpu_walk
+    n = 60000
+    pos = W.nfw(n, seed=4)
+    eps = 2.0 ** -8
+    g, v = gpu_build(pos, group_size=G)
+    aold = _bootstrap_aold(g, n, eps)
+    active = W.random_active_subset(n, frac, seed=11)
+    out, cnt, _ = gpu_walk(g, n, eps=eps, mac_kind=0, mac_param=2.0 ** -9, aold=aold, active=active)
+    ref, c = _oracle_on_gpu_tree(oracle, v, eps=eps, mac_kind=0, mac_param=2.0 ** -9, aold=aold, active=active, group_size=G)
+    assert cnt == c["interactions"]
+    _assert_parity(out, ref, active)
+    mask = np.ones(n, bool)
+    mask[active] = False
+    assert np.all(out[mask] == 0)     # only active entries written
+    # device-side count (no host round trip): same result
+    nad = torch.tensor([active.shape[0]], dtype=torch.int32, device="cuda")
+    padded = np.concatenate([active, np.zeros(100, np.uint32)])
+    out2, cnt2, _ = gpu_walk(g, n, eps=eps, mac_kind=0, mac_param=2.0 ** -9, aold=aold, active=padded, n_active_dev=nad)
+    assert cnt2 == cnt and np.array_equal(out2[active], out[active])
+    g.close()
+
+
+def test_walk_with_nothing_accepted_equals_direct_sum(oracle):
+    """Delta_acc = 0: the walk degenerates to eq. 1; fp32 accumulation => 1e-5."""
+    from gpu_util import gpu_build, gpu_walk, acc_rel_err
+    n = 3000
+    pos = W.plummer(n, seed=9)
+    g, v = gpu_build(pos, n_leaf=8)
+    eps = 1.0 / 64
+    ref = oracle.direct(v["pos_m_sorted"], eps)
+    for kind, aold in ((0, np.ones(n, np.float32)), (1, None)):
+        out, cnt, _ = gpu_walk(g, n, eps=eps, mac_kind=kind, mac_param=0.0, aold=aold)
+        assert cnt == n * n
+        e = acc_rel_err(out, ref)   # fp32 sum of 3000 terms; near the centre the terms cancel, so the worst particle is looser
+        assert np.percentile(e, 99) < 1e-5 and e.max() < 1e-4
+        assert (np.abs(out[:, 3] - ref[:, 3]) / np.abs(ref[:, 3])).max() < 1e-5
+    g.close()
+
+
+def test_walk_tiny_cases(oracle):
+    from gpu_util import gpu_build, gpu_walk
+    # two bodies: textbook softened force
+    m1, m2, d, eps = 2.0, 3.0, 1.5, 0.25
+    pos = np.array([[0, 0, 0, m1], [d, 0, 0, m2]], np.float32)
+    g, v = gpu_build(pos)
+    out, cnt, _ = gpu_walk(g, 2, eps=eps, mac_kind=1, mac_param=0.5)
+    s = d * d + eps * eps
+    o = out[np.argsort(v["perm"])]
+    assert o[0] == pytest.approx([m2 * d / s ** 1.5, 0, 0, -m2 / s ** 0.5], rel=2e-6, abs=1e-7)
+    assert o[1] == pytest.approx([-m1 * d / s ** 1.5, 0, 0, -m1 / s ** 0.5], rel=2e-6, abs=1e-7)
+    g.close()
+    # single particle: no force, zero potential
+    g, v = gpu_build(np.array([[1, 2, 3, 1]], np.float32))
+    out, cnt, _ = gpu_walk(g, 1, eps=0.1, mac_kind=1, mac_param=0.5)
+    assert np.all(out[0, :3] == 0) and abs(out[0, 3]) < 1e-6
+    g.close()
+    # coincident particles (level-21 leaf with num > n_leaf): finite, equals direct sum
+    pos = W.plummer(2000, seed=3)
+    pos[50:90, :3] = pos[50, :3]
+    g, v = gpu_build(pos)
+    out, _, _ = gpu_walk(g, 2000, eps=0.05, mac_kind=1, mac_param=0.0)
+    ref = oracle.direct(v["pos_m_sorted"], 0.05)
+    assert np.all(np.isfinite(out)) and np.abs(out - ref).max() < 1e-4 * np.abs(ref).max()
+    g.close()
+
+
+def test_walk_end_to_end_tolerances_and_error_vs_direct(oracle):
+    """BASELINE.json configs[0] (Plummer 2^13, eps 1/64, Delta_acc 2^-7) end to end: the oracle builds its OWN tree
+    and moments; MAC flips at threshold are allowed by the stated tolerances."""
+    from gpu_util import gpu_build, gpu_walk, acc_rel_err
+    pos, cfg = W.make_config("plummer_2p13", seed=1)
+    n, eps = cfg["n"], cfg["eps"]
+    g, v = gpu_build(pos)
+    t = oracle.build_tree(pos)
+    boot, _ = oracle.walk_tree(t, eps=eps, mac_kind=1, mac_param=0.5)
+    aold = np.linalg.norm(boot[:, :3], axis=1).astype(np.float32)
+    ref, c = oracle.walk_tree(t, eps=eps, mac_kind=0, mac_param=cfg["delta_acc"], aold=aold)
+    out, cnt, _ = gpu_walk(g, n, eps=eps, mac_kind=0, mac_param=cfg["delta_acc"], aold=aold)
+    _assert_parity(out, ref, np.arange(n))
+    assert abs(cnt - c["interactions"]) <= 1e-3 * c["interactions"]
+    direct = oracle.direct(t.pos_sorted, eps)
+    assert 3e-4 < np.median(acc_rel_err(out, direct)) < 3e-3   # ~1e-3 at Delta_acc = 2^-7
+    g.close()
+
+
+def test_walk_full_size_hernquist_sampled(oracle):
+    """BASELINE.json configs[1] at full size (N = 2^20) in the bench launch configuration; the oracle walks a
+    sample of groups on the GPU-built tree, all sampled particles compared one by one."""
+    from gpu_util import gpu_build, gpu_walk
+    pos, cfg = W.make_config("hernquist_2p20", seed=1)
+    n, eps = cfg["n"], cfg["eps"]
+    g, v = gpu_build(pos)
+    aold = _bootstrap_aold(g, n, eps)
+    out, cnt, _ = gpu_walk(g, n, eps=eps, mac_kind=0, mac_param=cfg["delta_acc"], aold=aold)
+    n_groups = n // 32
+    for lo in (0, n_groups // 2 - 100, n_groups - 200):
+        ref, c = _oracle_on_gpu_tree(oracle, v, eps=eps, mac_kind=0, mac_param=cfg["delta_acc"], aold=aold, group_range=(lo, lo + 200))
+        rows = np.arange(lo * 32, (lo + 200) * 32)
+        _assert_parity(out, ref, rows)
+    # physics at any size: momentum near-conservation and a bound potential
+    m = v["pos_m_sorted"][:, 3].astype(np.float64)
+    mom = np.linalg.norm((m[:, None] * out[:, :3]).sum(0)) / (m * np.linalg.norm(out[:, :3], axis=1)).sum()
+    assert mom < 2e-3 and np.all(out[:, 3] < 0)
+    assert 1000 < cnt / n < 2500
+    g.close()
