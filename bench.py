@@ -1,0 +1,436 @@
+#!/usr/bin/env python
+"""bench.py -- whole-hot-path benchmark of the B200-native GOTHIC block-step cycle (driver contract).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME] [--n N]
+
+A "step" is one full block-step CYCLE of the workload (BASELINE.json configs[2], NFW sphere N = 2^24 by default):
+    gothic_build_tree                                  (B1-B6: bbox, keys, sort, gather, nodes, moments)
+    gothic_set_timesteps(acc)                          (T1: block levels from the current accelerations)
+    for substep = 1 .. 2^(n_levels-1):
+        gothic_set_timesteps(substep)                  (T2: ascending active list, count stays on the device)
+        gothic_update_moments                          (B6 again: the paper recomputes pseudo-j every step)
+        gothic_walk_tree(active, |a_old|, Delta_acc)   (W1-W6)
+Positions are static (the configs carry no velocities), so the last substep (all particles active) refreshes every
+acceleration and the next cycle starts from it.  `value` = interactions of the cycle / device time of the cycle,
+inputs resident in HBM.  `e2e` = the same cycle through gothic_block_cycle_host with pinned HOST buffers (H2D of
+positions + previous accelerations and D2H of the result inside the timed region).
+Interactions are counted in a separate, identical, untimed replay ("in a separate run").
+
+N > 1 (torchrun): the path is single-GPU by design (BASELINE.json north_star: "one GPU only"), so every rank runs an
+independent replica (its own seed); no data-path collective; time = max over ranks; value = sum of interactions / time.
+
+--impl reference: times the CPU oracle (oracle/, as it stands) on the host cores on a bounded sample of the same
+workload; rank 0 only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "tree_walk_interactions_per_s_block_cycle"
+UNIT = "interactions/s"
+FLOP_PER_INTERACTION = 24          # 20 + rsqrt counted as 4 (the paper's GTX TITAN X convention); 20 and 28 also reported
+THETA_BOOTSTRAP = 0.5              # DESIGN.md R7
+ETA, MAX_LEVELS = 0.5, 8           # BASELINE.json configs[2]
+
+
+def _peaks() -> dict:
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        d["source"] = "measured"
+        return d
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "sm_max_mhz": 1965.0, "source": "fallback"}
+
+
+class ClockSampler:
+    """Samples SM clock / throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.max_mhz, self.power = [], set(), None, []
+        self._stop = threading.Event()
+        self._t = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nv = pynvml
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self._nv = None
+
+    def _run(self):
+        nv = self._nv
+        names = {"hw_slowdown": nv.nvmlClocksThrottleReasonHwSlowdown, "hw_thermal_slowdown": nv.nvmlClocksThrottleReasonHwThermalSlowdown,
+                 "sw_thermal_slowdown": nv.nvmlClocksThrottleReasonSwThermalSlowdown, "sw_power_cap": nv.nvmlClocksThrottleReasonSwPowerCap}
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM)))
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self._h) / 1000.0)
+                r = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self._h))
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            self._stop.wait(0.05)
+
+    def __enter__(self):
+        if self._nv is not None:
+            self._t = threading.Thread(target=self._run, daemon=True)
+            self._t.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._t is not None:
+            self._t.join()
+
+    def summary(self) -> dict:
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "power_w_max": max(self.power) if self.power else None, "samples": len(self.samples)}
+
+
+# ------------------------------------------------------------------------------------------------------------
+def run_reference(args, rank: int, world: int):
+    """The CPU oracle, as it stands, on the host cores: a bounded sample of the workload's all-active substep."""
+    if rank != 0:
+        return
+    import oracle
+    from paper_1610_07279_b200 import workloads as W
+    t0 = time.time()
+    pos, cfg = W.make_config(args.workload, seed=args.seed, n=args.n)
+    n, eps, dacc = cfg["n"], cfg["eps"], cfg["delta_acc"]
+    t_gen = time.time() - t0
+    t0 = time.time()
+    tree = oracle.build_tree(pos)
+    t_build = time.time() - t0
+    G = 32
+    n_groups = (n + G - 1) // G
+    cores = oracle.num_threads()
+    ranges = _sample_ranges(n_groups, args.ref_groups, 8)
+    # |a_old| for the sample: the oracle's own opening-angle bootstrap on the same groups (R7)
+    aold = np.ones(n, np.float32)
+    for lo, hi in ranges:
+        o, _ = oracle.walk_tree(tree, eps=eps, mac_kind=1, mac_param=THETA_BOOTSTRAP, group_range=(lo, hi))
+        aold[lo * G:hi * G] = np.linalg.norm(o[lo * G:hi * G, :3], axis=1).astype(np.float32)
+
+    def step():
+        cnt = 0
+        for lo, hi in ranges:
+            _, c = oracle.walk_tree(tree, eps=eps, mac_kind=0, mac_param=dacc, aold=aold, group_range=(lo, hi))
+            cnt += c["interactions"]
+        return cnt
+
+    for _ in range(args.warmup):
+        step()
+    t0 = time.time()
+    inter = 0
+    for _ in range(args.steps):
+        inter += step()
+    dt = time.time() - t0
+    val = inter / dt
+    sample = (f"{sum(hi - lo for lo, hi in ranges)} of {n_groups} i-groups (8 evenly spaced runs) of the all-active substep, "
+              f"fp64 accumulation, {inter // args.steps} interactions per step; oracle tree build {t_build:.1f} s (untimed)")
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": {"workload": args.workload, "n": n, "eps": eps, "delta_acc": dacc, "seed": args.seed},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0, "setup_s": {"generate": t_gen, "oracle_build": t_build}}
+    print(json.dumps(line), flush=True)
+
+
+def _sample_ranges(n_groups: int, want: int, pieces: int):
+    want = max(pieces, min(want, n_groups))
+    per = max(1, want // pieces)
+    out = []
+    for k in range(pieces):
+        lo = min(n_groups - per, (n_groups * k) // pieces)
+        lo = max(lo, out[-1][1] if out else 0)
+        hi = min(n_groups, lo + per)
+        if hi > lo:
+            out.append((lo, hi))
+    return out
+
+
+def cpu_baseline(pos, cfg, budget_s: float = 15.0) -> dict:
+    """Oracle walk (fp64 sum, OpenMP over groups) on a sample of the all-active substep sized to ~budget_s."""
+    import oracle
+    n, eps, dacc = cfg["n"], cfg["eps"], cfg["delta_acc"]
+    t0 = time.time()
+    tree = oracle.build_tree(pos)
+    t_build = time.time() - t0
+    G = 32
+    n_groups = (n + G - 1) // G
+    cores = oracle.num_threads()
+
+    def run(ranges):
+        aold = np.ones(n, np.float32)
+        for lo, hi in ranges:
+            o, _ = oracle.walk_tree(tree, eps=eps, mac_kind=1, mac_param=THETA_BOOTSTRAP, group_range=(lo, hi))
+            aold[lo * G:hi * G] = np.linalg.norm(o[lo * G:hi * G, :3], axis=1).astype(np.float32)
+        t0 = time.time()
+        cnt = 0
+        for lo, hi in ranges:
+            _, c = oracle.walk_tree(tree, eps=eps, mac_kind=0, mac_param=dacc, aold=aold, group_range=(lo, hi))
+            cnt += c["interactions"]
+        return cnt, time.time() - t0
+
+    probe = _sample_ranges(n_groups, 64 * cores, 8)
+    cnt, dt = run(probe)
+    want = int(sum(hi - lo for lo, hi in probe) * (budget_s / 2.2) / max(dt, 1e-3))   # bootstrap + MAC walk ~ 2.2 x the timed part
+    ranges = _sample_ranges(n_groups, want, 8)
+    cnt, dt = run(ranges)
+    ng = sum(hi - lo for lo, hi in ranges)
+    return {"value": cnt / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{ng} of {n_groups} i-groups (8 evenly spaced runs) of the all-active substep, fp64 accumulation, {cnt} interactions in "
+                      f"{dt:.2f} s; oracle tree build at full N took {t_build:.1f} s (not in the rate)"}
+
+
+# ------------------------------------------------------------------------------------------------------------
+def run_ours(args, rank: int, world: int, local_rank: int):
+    import torch
+    from paper_1610_07279_b200 import workloads as W
+    from paper_1610_07279_b200.binding import Gothic, MAC_ACCELERATION, MAC_OPENING_ANGLE
+
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    peaks = _peaks()
+    pos_np, cfg = W.make_config(args.workload, seed=args.seed + rank, n=args.n)
+    n, eps, dacc = cfg["n"], cfg["eps"], cfg["delta_acc"]
+    block = cfg["block"]
+    props = torch.cuda.get_device_properties(dev)
+
+    g = Gothic(n)
+    pos_host = torch.from_numpy(pos_np).pin_memory()
+    pos = pos_host.to(dev, non_blocking=True)
+    acc = torch.zeros(n, 4, dtype=torch.float32, device=dev)
+    amag = torch.zeros(n, dtype=torch.float32, device=dev)
+    level = torch.zeros(n, dtype=torch.uint8, device=dev)
+    active = torch.zeros(n, dtype=torch.int32, device=dev)
+    n_act = torch.zeros(1, dtype=torch.int32, device=dev)
+    emin_nlev = torch.zeros(2, dtype=torch.int32, device=dev)
+    counter = torch.zeros(1, dtype=torch.int64, device=dev)
+
+    # ---- untimed bootstrap (R7): opening-angle walk -> |a_old|, then one acceleration-MAC walk -------------
+    g.build_tree(pos)
+    g.walk_tree(acc, eps=eps, mac_kind=MAC_OPENING_ANGLE, mac_param=THETA_BOOTSTRAP, amag_out=amag)
+    g.walk_tree(acc, eps=eps, mac_kind=MAC_ACCELERATION, mac_param=dacc, aold=amag, amag_out=amag)
+    if block:
+        g.set_timesteps(level, acc_pot=acc, eps=eps, eta=ETA, max_levels=MAX_LEVELS, emin_nlev_dev=emin_nlev)
+        g.check()
+        e_min, n_levels = (int(x) for x in emin_nlev.tolist())
+    else:
+        e_min, n_levels = 0, 1
+    n_sub = 1 << (n_levels - 1)
+
+    stage_names = ["build", "levels", "active", "moments", "walk"]
+
+    def cycle(ev=None, counts=None):
+        """One step.  ev: optional list collecting (stage, start_event, stop_event); counts: per-substep interaction tensor."""
+        def timed(name, fn):
+            if ev is None:
+                fn()
+                return
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            fn()
+            b.record()
+            ev.append((name, a, b))
+        timed("build", lambda: g.build_tree(pos))
+        if block:
+            timed("levels", lambda: g.set_timesteps(level, acc_pot=acc, eps=eps, eta=ETA, max_levels=MAX_LEVELS, emin_nlev_dev=emin_nlev))
+        for s in range(1, n_sub + 1):
+            if block:
+                timed("active", lambda: g.set_timesteps(level, acc_pot=None, eps=eps, substep=s, active=active, n_active_dev=n_act))
+                timed("moments", lambda: g.update_moments())
+                timed("walk", lambda: g.walk_tree(acc, eps=eps, mac_kind=MAC_ACCELERATION, mac_param=dacc, aold=amag, active=active,
+                                                   n_active_dev=n_act, amag_out=amag,
+                                                   n_interactions=None if counts is None else counts[s - 1:s]))
+            else:
+                timed("walk", lambda: g.walk_tree(acc, eps=eps, mac_kind=MAC_ACCELERATION, mac_param=dacc, aold=amag, amag_out=amag,
+                                                   n_interactions=None if counts is None else counts[s - 1:s]))
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        cycle()
+    g.check()
+    snap = (acc.clone(), amag.clone(), level.clone())
+
+    # ---- timed region: exactly K steps -------------------------------------------------------------------------------
+    launches0 = g.launch_count()
+    ev = []
+    t_start, t_stop = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    with ClockSampler(local_rank) as clk:
+        t_start.record()
+        for _ in range(args.steps):
+            cycle(ev)
+        t_stop.record()
+        barrier()
+    total_ms = t_start.elapsed_time(t_stop)
+    launches = g.launch_count() - launches0
+    g.check()
+    stage_ms = {k: 0.0 for k in stage_names}
+    walk_ms_sub = np.zeros(n_sub)
+    wi = 0
+    for name, a, b in ev:
+        ms = a.elapsed_time(b)
+        stage_ms[name] += ms
+        if name == "walk":
+            walk_ms_sub[wi % n_sub] += ms
+            wi += 1
+    walk_launches = wi
+
+    # ---- identical untimed replay with the interaction counter on ----------------------------------------------
+    acc.copy_(snap[0]); amag.copy_(snap[1]); level.copy_(snap[2])
+    counts = torch.zeros(n_sub, dtype=torch.int64, device=dev)
+    act_counts = np.zeros(n_sub, np.int64)
+    inter_sub = np.zeros(n_sub, np.int64)
+    for _ in range(args.steps):
+        counts.zero_()
+        cycle(None, counts)
+        inter_sub += counts.cpu().numpy()
+    if block:   # active counts per substep (same every cycle: levels are recomputed from converged accelerations)
+        for s in range(1, n_sub + 1):
+            g.set_timesteps(level, acc_pot=None, eps=eps, substep=s, active=active, n_active_dev=n_act)
+            act_counts[s - 1] = int(n_act.item())
+    else:
+        act_counts[:] = n
+    inter_total = int(inter_sub.sum())
+
+    # ---- e2e: same cycle through the host-buffer C-ABI call ---------------------------------------------------------------
+    e2e = None
+    if block:
+        k_e2e = max(1, min(args.steps, 3))
+        acc_prev_sorted = snap[0]
+        perm = g.get_tree_view()["perm"].long()
+        acc_prev_orig = torch.empty_like(acc_prev_sorted)
+        acc_prev_orig[perm] = acc_prev_sorted
+        h_prev = acc_prev_orig.cpu().pin_memory()
+        h_prev0 = h_prev.clone().pin_memory()
+        h_out = torch.empty(n, 4, dtype=torch.float32).pin_memory()
+        h_lev = torch.empty(n, dtype=torch.uint8).pin_memory()
+        del acc_prev_orig, perm
+        g.block_cycle_host(pos_host, h_prev, h_out, eps=eps, delta_acc=dacc, eta=ETA, max_levels=MAX_LEVELS, level_host=h_lev)   # warm-up
+        h_prev.copy_(h_prev0)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        t0 = time.perf_counter()
+        e0.record()
+        a, b = h_prev, h_out
+        for _ in range(k_e2e):
+            g.block_cycle_host(pos_host, a, b, eps=eps, delta_acc=dacc, eta=ETA, max_levels=MAX_LEVELS, level_host=h_lev)
+            a, b = b, a
+        e1.record()
+        barrier()
+        e2e_wall_ms = 1e3 * (time.perf_counter() - t0)
+        e2e_ms = max(e0.elapsed_time(e1), e2e_wall_ms)     # host-synchronous call: wall clock covers the copies too
+        # counted replay
+        h_prev.copy_(h_prev0)
+        a, b, e2e_inter = h_prev, h_out, 0
+        for _ in range(k_e2e):
+            info = g.block_cycle_host(pos_host, a, b, eps=eps, delta_acc=dacc, eta=ETA, max_levels=MAX_LEVELS, level_host=h_lev, count=True)
+            e2e_inter += info["interactions"]
+            a, b = b, a
+        e2e = {"ms": e2e_ms, "steps": k_e2e, "interactions": e2e_inter, "h2d": 2 * n * 16, "d2h": n * 16 + n}
+
+    # ---- max over ranks, aggregate ---------------------------------------------------------------------------------------
+    t_all = torch.tensor([total_ms, stage_ms["walk"], e2e["ms"] if e2e else 0.0], dtype=torch.float64, device=dev)
+    i_all = torch.tensor([inter_total, e2e["interactions"] if e2e else 0], dtype=torch.int64, device=dev)
+    if dist is not None:
+        dist.all_reduce(t_all, op=dist.ReduceOp.MAX)
+        dist.all_reduce(i_all, op=dist.ReduceOp.SUM)
+    total_ms_max, walk_ms_max, e2e_ms_max = (float(x) for x in t_all.tolist())
+    inter_all, e2e_inter_all = (int(x) for x in i_all.tolist())
+
+    if rank == 0:
+        K = args.steps
+        value = inter_all / (total_ms_max * 1e-3)
+        walk_rate = inter_total / (stage_ms["walk"] * 1e-3)            # this rank's walk stage
+        alu_peak = props.multi_processor_count * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12      # TFLOP/s, DESIGN.md "Rooflines"
+        achieved = walk_rate * FLOP_PER_INTERACTION / 1e12
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
+            "ms_per_step": total_ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": args.workload, "n": n, "eps": eps, "delta_acc": dacc, "eta": ETA, "max_levels": MAX_LEVELS, "seed": args.seed,
+                       "group_size": 32, "n_leaf": 16, "key": "peano_hilbert", "n_levels": n_levels, "n_substeps": n_sub,
+                       "parallelism": "replicas" if world > 1 else "single_gpu", "l2": "inputs_exceed_l2" if n * 16 > 126e6 else "inputs_fit_l2"},
+            "sec_per_block_step": total_ms_max * 1e-3 / K / n_sub,
+            "interactions_per_cycle": inter_total // K,
+            "stage_ms_per_cycle": {k: v / K for k, v in stage_ms.items()},
+            "substeps": [{"substep": s + 1, "n_active": int(act_counts[s]), "interactions": int(inter_sub[s] // K),
+                          "walk_ms": walk_ms_sub[s] / K,
+                          "interactions_per_s": float(inter_sub[s] / max(walk_ms_sub[s], 1e-9) * 1e3)} for s in range(n_sub)],
+            "walk": {"interactions_per_s": walk_rate, "tflops_20": walk_rate * 20 / 1e12, "tflops_24": walk_rate * 24 / 1e12,
+                     "tflops_28": walk_rate * 28 / 1e12, "frac_fp32_peak_24": achieved / alu_peak},
+            "roofline": {"kernel": "k_walk", "bound": "alu", "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s", "frac": achieved / alu_peak,
+                         "traffic": None, "flop_per_interaction": FLOP_PER_INTERACTION,
+                         "avg_launch_ms": stage_ms["walk"] / max(walk_launches, 1),
+                         "peak_source": f"derived: {props.multi_processor_count} SM x 128 FP32 lanes x 2 flop x {peaks['sm_max_mhz']:.0f} MHz "
+                                        f"(clock from MEASURED_PEAKS.json, {peaks['source']})"},
+            "clocks": clk.summary(),
+            "gpu_launches": int(launches),
+            "e2e": None,
+        }
+        if e2e:
+            line["e2e"] = {"value": e2e_inter_all / (e2e_ms_max * 1e-3), "unit": UNIT, "h2d_bytes_per_step": e2e["h2d"],
+                           "d2h_bytes_per_step": e2e["d2h"], "ms_per_step": e2e_ms_max / e2e["steps"], "steps": e2e["steps"]}
+        if world == 1 and not args.no_cpu_baseline:
+            del g
+            line["cpu_baseline"] = cpu_baseline(pos_np, cfg, args.cpu_budget)
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="nfw_2p24_block")
+    ap.add_argument("--n", type=int, default=None, help="override N (debugging; the reported config then says so)")
+    ap.add_argument("--seed", type=int, default=1)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-budget", type=float, default=15.0)
+    ap.add_argument("--ref-groups", type=int, default=65536, help="i-groups per step of the --impl reference sample")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

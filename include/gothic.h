@@ -130,6 +130,22 @@ int gothic_gravity_host(gothic_ctx *ctx, const float *pos_m_host, uint32_t n, in
                         float eps, int mac_kind, float mac_param, const float *aold_host,
                         float *acc_pot_host, uint32_t *perm_host, void *stream);
 
+/* One full block-step cycle end to end with HOST buffers (bench.py "e2e"; the paper's per-step loop PAPER.md:179-187
+ * with static positions): H2D copy of pos_m and of the previous accelerations, tree build, block levels from the
+ * previous accelerations (gothic_set_timesteps), then for substep = 1 .. 2^(n_levels-1): active list, pseudo-j moments
+ * (recomputed every step), walk of the active particles with the acceleration MAC (eq. 5) using the
+ * running |a| as |a_old|; finally D2H copy of the accelerations.  The last substep has every particle active, so
+ * acc_pot_host is complete.  Synchronises (one small read-back of n_levels, one at the end).
+ *   pos_m_host    float4[n] HOST (pinned for full speed), ORIGINAL order.
+ *   acc_prev_host float4[n] HOST, ORIGINAL order: accelerations of the previous step (levels and |a_old|, R6/R7).
+ *   acc_pot_host  float4[n] HOST out, ORIGINAL order.   level_host  uint8[n] HOST out, ORIGINAL order (may be NULL).
+ *   info_host     int32[4] HOST out: {exponent of finest dt, n_levels, n_substeps, 0} (may be NULL).
+ *   n_interactions_host  optional HOST out: interactions summed over the cycle (enables the device counter;
+ *                        pass NULL in timed runs). */
+int gothic_block_cycle_host(gothic_ctx *ctx, const float *pos_m_host, const float *acc_prev_host, uint32_t n, int key_kind,
+                            int n_leaf, float eps, float eta, int max_levels, float delta_acc, float *acc_pot_host,
+                            uint8_t *level_host, int32_t *info_host, unsigned long long *n_interactions_host, void *stream);
+
 /* Number of kernels this library has launched through this context (bench.py "gpu_launches"). */
 unsigned long long gothic_launch_count(gothic_ctx *ctx);
 

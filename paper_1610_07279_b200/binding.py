@@ -19,7 +19,7 @@ MAC_ACCELERATION, MAC_OPENING_ANGLE = 0, 1
 EXPORTS = [
     "gothic_create", "gothic_destroy", "gothic_strerror", "gothic_last_cuda_error", "gothic_build_tree",
     "gothic_update_moments", "gothic_walk_tree", "gothic_set_timesteps", "gothic_get_tree_view", "gothic_check",
-    "gothic_gravity_host", "gothic_launch_count",
+    "gothic_gravity_host", "gothic_block_cycle_host", "gothic_launch_count",
 ]
 
 
@@ -70,6 +70,8 @@ def load_library():
     L.gothic_check.argtypes = [vp, vp]
     L.gothic_gravity_host.restype = i32
     L.gothic_gravity_host.argtypes = [vp, vp, u32, i32, i32, f32, i32, f32, vp, vp, vp, vp]
+    L.gothic_block_cycle_host.restype = i32
+    L.gothic_block_cycle_host.argtypes = [vp, vp, vp, u32, i32, i32, f32, f32, i32, f32, vp, vp, vp, vp, vp]
     L.gothic_launch_count.restype = C.c_ulonglong
     L.gothic_launch_count.argtypes = [vp]
     _lib = L
@@ -194,3 +196,18 @@ class Gothic:
         hp = lambda t: None if t is None else C.c_void_p(t.data_ptr())
         self._chk(self._L.gothic_gravity_host(self._ctx, hp(pos_m_host), pos_m_host.shape[0], key_kind, n_leaf, float(eps), mac_kind,
                                               float(mac_param), hp(aold_host), hp(acc_pot_host), hp(perm_host), _stream()))
+
+    def block_cycle_host(self, pos_m_host: torch.Tensor, acc_prev_host: torch.Tensor, acc_pot_host: torch.Tensor, *, eps: float,
+                         delta_acc: float, eta: float = 0.5, max_levels: int = 8, level_host: torch.Tensor | None = None,
+                         count: bool = False, key_kind: int = KEY_PEANO_HILBERT, n_leaf: int = 16) -> dict:
+        """One full block-step cycle end to end with HOST (pinned) buffers: H2D, build, levels, all substeps, D2H."""
+        for t in (pos_m_host, acc_prev_host, acc_pot_host, level_host):
+            if t is not None and (t.is_cuda or not t.is_contiguous()):
+                raise GothicError("block_cycle_host expects contiguous host tensors")
+        hp = lambda t: None if t is None else C.c_void_p(t.data_ptr())
+        info = (C.c_int32 * 4)()
+        cnt = C.c_ulonglong(0)
+        self._chk(self._L.gothic_block_cycle_host(self._ctx, hp(pos_m_host), hp(acc_prev_host), pos_m_host.shape[0], key_kind, n_leaf,
+                                                  float(eps), float(eta), max_levels, float(delta_acc), hp(acc_pot_host), hp(level_host),
+                                                  C.cast(info, C.c_void_p), C.cast(C.pointer(cnt), C.c_void_p) if count else None, _stream()))
+        return dict(e_min=info[0], n_levels=info[1], n_substeps=info[2], interactions=int(cnt.value) if count else None)

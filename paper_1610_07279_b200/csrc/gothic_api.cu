@@ -18,7 +18,8 @@ void free_all(gothic_ctx *c)
                     c->node_head, c->node_num, c->node_child, c->node_parent, c->node_end, c->node_last,
                     c->node_level, c->node_nchild, c->node_com, c->node_msum, c->node_b, c->node_b2bits, c->node_rec,
                     c->level_ofs, c->level_cnt, c->blk_cnt, c->flags, c->sort_tmp, c->grp_mask, c->grp_list, c->grp_cnt,
-                    c->stack, c->ts_tmp, c->scan_tmp, c->h2d_pos, c->h2d_aold, c->d_aold_sorted, c->d_acc};
+                    c->stack, c->ts_tmp, c->scan_tmp, c->h2d_pos, c->h2d_aold, c->d_aold_sorted, c->d_acc,
+                    c->h2d_acc, c->d_level, c->d_active, c->d_cycle_info, c->d_count};
     for (void *p : ptrs)
         if (p) cudaFree(p);
 }
@@ -27,6 +28,28 @@ __global__ void k_gather_f32(const float *__restrict__ src, const uint32_t *__re
 {
     const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s < n) dst[s] = __ldg(src + __ldg(perm + s));
+}
+
+// sorted <- original: acc_sorted[s] = acc_orig[perm[s]], amag[s] = |a|
+__global__ void k_gather_acc(const float4 *__restrict__ src, const uint32_t *__restrict__ perm, uint32_t n, float4 *__restrict__ dst,
+                             float *__restrict__ amag)
+{
+    const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n) return;
+    const float4 a = __ldg(src + __ldg(perm + s));
+    dst[s] = a;
+    amag[s] = __fsqrt_rn(fmaf(a.z, a.z, fmaf(a.y, a.y, a.x * a.x)));
+}
+
+// original <- sorted: acc_orig[perm[s]] = acc_sorted[s], level_orig[perm[s]] = level_sorted[s]
+__global__ void k_scatter_result(const float4 *__restrict__ acc_sorted, const uint8_t *__restrict__ level_sorted,
+                                 const uint32_t *__restrict__ perm, uint32_t n, float4 *__restrict__ acc_orig, uint8_t *__restrict__ level_orig)
+{
+    const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n) return;
+    const uint32_t o = __ldg(perm + s);
+    acc_orig[o] = acc_sorted[s];
+    level_orig[o] = level_sorted[s];
 }
 
 } // namespace
@@ -251,6 +274,67 @@ int gothic_gravity_host(gothic_ctx *c, const float *pos_m_host, uint32_t n, int 
     GOTHIC_CUDA_OK(c, cudaMemcpyAsync(acc_pot_host, c->d_acc, (size_t)n * sizeof(float4), cudaMemcpyDeviceToHost, s));
     if (perm_host)
         GOTHIC_CUDA_OK(c, cudaMemcpyAsync(perm_host, c->idx[c->cur], (size_t)n * sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
+    return gothic_check(c, stream);
+}
+
+int gothic_block_cycle_host(gothic_ctx *c, const float *pos_m_host, const float *acc_prev_host, uint32_t n, int key_kind, int n_leaf,
+                            float eps, float eta, int max_levels, float delta_acc, float *acc_pot_host, uint8_t *level_host,
+                            int32_t *info_host, unsigned long long *n_interactions_host, void *stream)
+{
+    if (!c || !pos_m_host || !acc_prev_host || !acc_pot_host || n == 0 || n > c->n_max) return GOTHIC_ERR_ARG;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    if (!c->h2d_pos) {
+        cudaError_t e = dev_alloc(&c->h2d_pos, c->n_max);
+        if (e == cudaSuccess) e = dev_alloc(&c->h2d_aold, c->n_max);
+        if (e == cudaSuccess) e = dev_alloc(&c->d_aold_sorted, c->n_max);
+        if (e == cudaSuccess) e = dev_alloc(&c->d_acc, c->n_max);
+        if (e != cudaSuccess) { c->last_err = e; return GOTHIC_ERR_CUDA; }
+    }
+    if (!c->h2d_acc) {
+        cudaError_t e = dev_alloc(&c->h2d_acc, c->n_max);
+        if (e == cudaSuccess) e = dev_alloc(&c->d_level, 2 * (size_t)c->n_max);
+        if (e == cudaSuccess) e = dev_alloc(&c->d_active, c->n_max);
+        if (e == cudaSuccess) e = dev_alloc(&c->d_cycle_info, 4);
+        if (e == cudaSuccess) e = dev_alloc(&c->d_count, 1);
+        if (e != cudaSuccess) { c->last_err = e; return GOTHIC_ERR_CUDA; }
+    }
+    const size_t b4 = (size_t)n * sizeof(float4);
+    GOTHIC_CUDA_OK(c, cudaMemcpyAsync(c->h2d_pos, pos_m_host, b4, cudaMemcpyHostToDevice, s));
+    GOTHIC_CUDA_OK(c, cudaMemcpyAsync(c->h2d_acc, acc_prev_host, b4, cudaMemcpyHostToDevice, s));
+    int rc = gothic_build_tree(c, reinterpret_cast<const float *>(c->h2d_pos), n, key_kind, n_leaf, stream);
+    if (rc != GOTHIC_OK) return rc;
+    const uint32_t grid = (n + 255u) / 256u;
+    float *amag = c->d_aold_sorted;
+    uint8_t *level = c->d_level, *level_orig = c->d_level + c->n_max;
+    uint32_t *n_active_dev = reinterpret_cast<uint32_t *>(c->d_cycle_info) + 2;
+    k_gather_acc<<<grid, 256, 0, s>>>(c->h2d_acc, c->idx[c->cur], n, c->d_acc, amag);
+    GOTHIC_LAUNCH_OK(c);
+    rc = gothic_set_timesteps(c, reinterpret_cast<const float *>(c->d_acc), n, eps, eta, max_levels, 1u, level, nullptr, nullptr,
+                              c->d_cycle_info, stream);
+    if (rc != GOTHIC_OK) return rc;
+    int32_t emin_nlev[2];
+    GOTHIC_CUDA_OK(c, cudaMemcpyAsync(emin_nlev, c->d_cycle_info, sizeof(emin_nlev), cudaMemcpyDeviceToHost, s));
+    GOTHIC_CUDA_OK(c, cudaStreamSynchronize(s));
+    const int n_levels = emin_nlev[1];
+    if (n_levels < 1 || n_levels > max_levels) return GOTHIC_ERR_STATE;
+    const uint32_t n_sub = 1u << (n_levels - 1);
+    if (n_interactions_host) GOTHIC_CUDA_OK(c, cudaMemsetAsync(c->d_count, 0, sizeof(unsigned long long), s));
+    for (uint32_t sub = 1; sub <= n_sub; sub++) {
+        rc = gothic_set_timesteps(c, nullptr, n, eps, eta, max_levels, sub, level, c->d_active, n_active_dev, nullptr, stream);
+        if (rc != GOTHIC_OK) return rc;
+        rc = gothic_update_moments(c, nullptr, stream);   // the paper recomputes the pseudo j-particles every step
+        if (rc != GOTHIC_OK) return rc;
+        rc = gothic_walk_tree(c, c->d_active, 0, n_active_dev, eps, GOTHIC_MAC_ACCELERATION, delta_acc, amag,
+                              reinterpret_cast<float *>(c->d_acc), amag, n_interactions_host ? c->d_count : nullptr, stream);
+        if (rc != GOTHIC_OK) return rc;
+    }
+    k_scatter_result<<<grid, 256, 0, s>>>(c->d_acc, level, c->idx[c->cur], n, c->h2d_acc, level_orig);
+    GOTHIC_LAUNCH_OK(c);
+    GOTHIC_CUDA_OK(c, cudaMemcpyAsync(acc_pot_host, c->h2d_acc, b4, cudaMemcpyDeviceToHost, s));
+    if (level_host) GOTHIC_CUDA_OK(c, cudaMemcpyAsync(level_host, level_orig, n, cudaMemcpyDeviceToHost, s));
+    if (n_interactions_host)
+        GOTHIC_CUDA_OK(c, cudaMemcpyAsync(n_interactions_host, c->d_count, sizeof(unsigned long long), cudaMemcpyDeviceToHost, s));
+    if (info_host) { info_host[0] = emin_nlev[0]; info_host[1] = n_levels; info_host[2] = (int32_t)n_sub; info_host[3] = 0; }
     return gothic_check(c, stream);
 }
 
