@@ -54,7 +54,7 @@ def lib():
         L.oracle_walk.restype = None
         L.oracle_walk.argtypes = [_f32p, C.c_uint32, _u32p, _u32p, _u32p, _u8p, _f32p, _f32p,
                                   C.c_void_p, C.c_uint32, C.c_int, C.c_float, C.c_int, C.c_float, C.c_void_p,
-                                  C.c_uint32, C.c_uint32, _f64p, _u64p]
+                                  C.c_uint32, C.c_uint32, C.c_float, _f64p, _u64p]
         L.oracle_group_ball.restype = None
         L.oracle_group_ball.argtypes = [_f32p, _u32p, C.c_uint32, _f32p]
         _lib = L
@@ -212,8 +212,9 @@ def direct(pos_m, eps: float, targets=None) -> np.ndarray:
 
 
 def walk(pos_sorted, head, num, child, nchild, com, b, *, eps: float, mac_kind: int, mac_param: float,
-         aold=None, active=None, group_size: int = 32, group_range=None):
-    """O7.  Returns (out float64 [n,4] (only active rows written), counts dict)."""
+         aold=None, active=None, group_size: int = 32, group_range=None, r_crit: float = float("inf")):
+    """O7.  Returns (out float64 [n,4] (only active rows written), counts dict).
+    r_crit: critical separation of P:122-126 (reading R13); inf = no group splitting."""
     pos_sorted = _pos(pos_sorted)
     n = pos_sorted.shape[0]
     out = np.zeros((n, 4), np.float64)
@@ -235,7 +236,7 @@ def walk(pos_sorted, head, num, child, nchild, com, b, *, eps: float, mac_kind: 
                       np.ascontiguousarray(child, np.uint32), np.ascontiguousarray(nchild, np.uint8),
                       np.ascontiguousarray(com, np.float32), np.ascontiguousarray(b, np.float32),
                       act_p, n_act, group_size, float(eps), mac_kind, float(mac_param), aold_p,
-                      int(g_lo), int(g_hi), out, counts)
+                      int(g_lo), int(g_hi), float(r_crit), out, counts)
     return out, dict(interactions=int(counts[0]), mac_tests=int(counts[1]), groups=int(counts[2]), list_entries=int(counts[3]))
 
 

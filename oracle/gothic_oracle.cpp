@@ -30,6 +30,7 @@
 #include <cstdint>
 #include <cstring>
 #include <numeric>
+#include <utility>
 #include <vector>
 #ifdef _OPENMP
 #include <omp.h>
@@ -342,6 +343,8 @@ void oracle_direct(const float *pos_m, uint32_t n, const uint32_t *targets, uint
     }
 }
 
+void oracle_group_ball(const float *pos_sorted, const uint32_t *members, uint32_t k, float *ball4);
+
 /* O7 (P:105-118 traversal with a pseudo i-particle; eq. 5; eq. 2; P:62 monopole).
  * One group = aligned chunk of G consecutive sorted indices (reading R3); members = its active particles;
  * GEO enclosing ball and a_min = min |a_old| over members (R4).  All MAC-deciding arithmetic in fp32 with
@@ -350,13 +353,17 @@ void oracle_direct(const float *pos_m, uint32_t n, const uint32_t *targets, uint
  *   out4: double (ax, ay, az, Phi) for every sorted index (only active entries written).
  *   counts[0] += sum over groups |K| * |list|   (interactions, P:331 convention)
  *   counts[1] += MAC evaluations, counts[2] += groups walked, counts[3] += sum |list|
- *   group_lo/group_hi: only groups g with group_lo <= g < group_hi are walked (bounded samples). */
+ *   group_lo/group_hi: only groups g with group_lo <= g < group_hi are walked (bounded samples).
+ *   r_crit: "critical separation ... to judge whether to unify i-particles into a group or not" (§2.4).
+ *           The paper gives no formula; reading R13: a chunk's member list (ascending sorted index) whose GEO ball has
+ *           b_I > r_crit is cut into its first ceil(k/2) members and the rest, recursively, until b_I <= r_crit or one
+ *           member is left; every piece then walks the tree on its own.  r_crit = INFINITY: no splitting (R3 as is). */
 void oracle_walk(const float *pos_sorted, uint32_t n,
                  const uint32_t *head, const uint32_t *num, const uint32_t *child, const uint8_t *nchild,
                  const float *com4, const float *bJ,
                  const uint32_t *active, uint32_t n_active, int G,
                  float eps, int mac_kind, float mac_param, const float *aold,
-                 uint32_t group_lo, uint32_t group_hi,
+                 uint32_t group_lo, uint32_t group_hi, float r_crit,
                  double *out4, uint64_t *counts)
 {
     const uint32_t n_groups = (n + (uint32_t)G - 1) / (uint32_t)G;
@@ -379,6 +386,23 @@ void oracle_walk(const float *pos_sorted, uint32_t n,
             for (uint32_t s = (uint32_t)g * G; s < std::min(n, (uint32_t)(g + 1) * G); s++) K.push_back(s);
         }
         if (K.empty()) continue;
+        /* §2.4 / R13: pieces of the member list, produced depth-first (first half before second half) */
+        std::vector<std::pair<uint32_t, uint32_t>> todo(1, std::make_pair(0u, (uint32_t)K.size())), pieces;
+        while (!todo.empty()) {
+            const std::pair<uint32_t, uint32_t> pr = todo.back();
+            todo.pop_back();
+            const uint32_t cnt = pr.second - pr.first;
+            float ball[4];
+            oracle_group_ball(pos_sorted, K.data() + pr.first, cnt, ball);
+            if (cnt > 1 && ball[3] > r_crit) {
+                const uint32_t mid = pr.first + (cnt + 1) / 2;
+                todo.push_back(std::make_pair(mid, pr.second));
+                todo.push_back(std::make_pair(pr.first, mid));
+            } else pieces.push_back(pr);
+        }
+        const std::vector<uint32_t> Kall = K;
+        for (const std::pair<uint32_t, uint32_t> &pc : pieces) {
+        K.assign(Kall.begin() + pc.first, Kall.begin() + pc.second);
         /* pseudo i-particle: GEO ball (App. B P:568 item 3) */
         float lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
         float amin = INFINITY;
@@ -449,6 +473,7 @@ void oracle_walk(const float *pos_sorted, uint32_t n,
         c_int += (uint64_t)K.size() * L;
         c_list += L;
         c_grp++;
+        } /* pieces */
     }
     if (counts) { counts[0] += c_int; counts[1] += c_mac; counts[2] += c_grp; counts[3] += c_list; }
 }

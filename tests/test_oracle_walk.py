@@ -157,3 +157,106 @@ def test_plummer_closed_form_large_n(oracle):
         assert k > 300
         assert np.mean(a_r[sel]) == pytest.approx(np.mean(-mass(r[sel]) / r[sel] ** 2), rel=6.0 / np.sqrt(k))
         assert np.mean(out[sel, 3]) == pytest.approx(np.mean(phi(r[sel])), rel=0.02)
+
+
+# ---- group splitting by the critical separation r_crit (reading R13) ---------------------------------------
+def _pieces_numpy(pos_sorted, members, r_crit):
+    """Independent restatement of R13 in numpy float32: halve the member list while its GEO ball is wider than r_crit."""
+    p = pos_sorted[members, :3].astype(np.float32)
+    c = np.float32(0.5) * (p.min(0) + p.max(0))
+    d = p - c
+    b = np.sqrt(np.max(np.float32(d[:, 2] * d[:, 2]) + (np.float32(d[:, 1] * d[:, 1]) + np.float32(d[:, 0] * d[:, 0]))))
+    if len(members) > 1 and b > r_crit:
+        mid = (len(members) + 1) // 2
+        return _pieces_numpy(pos_sorted, members[:mid], r_crit) + _pieces_numpy(pos_sorted, members[mid:], r_crit)
+    return [members]
+
+
+@pytest.mark.parametrize("r_crit", [0.0, 0.05, 0.3, 1.0])
+def test_rcrit_split_equals_walking_each_piece_as_its_own_active_set(oracle, r_crit):
+    """A chunk walked with r_crit must give exactly what walking each piece of the R13 recursion separately gives
+    (pieces found by an independent numpy restatement), and as many traversals as there are pieces."""
+    n = 4000
+    pos = W.hernquist(n, seed=8)
+    t = oracle.build_tree(pos)
+    eps = 0.01
+    active = W.random_active_subset(n, 0.6, seed=2)
+    kw = dict(eps=eps, mac_kind=1, mac_param=0.7)
+    out, c = oracle.walk_tree(t, active=active, r_crit=r_crit, **kw)
+    n_pieces, inter = 0, 0
+    ref = np.zeros_like(out)
+    for g in range((n + 31) // 32):
+        members = active[(active >= 32 * g) & (active < 32 * g + 32)]
+        if members.size == 0:
+            continue
+        for piece in _pieces_numpy(t.pos_sorted, members, np.float32(r_crit)):
+            o, cc = oracle.walk_tree(t, active=piece, group_range=(g, g + 1), **kw)
+            ref[piece] = o[piece]
+            n_pieces += 1
+            inter += cc["interactions"]
+            ball = oracle.group_ball(t.pos_sorted, piece)
+            assert piece.size == 1 or ball[3] <= r_crit
+    assert c["groups"] == n_pieces and c["interactions"] == inter
+    assert np.array_equal(out, ref)
+    if r_crit == 0.0:
+        assert c["groups"] == active.size     # every member on its own: b_I = 0
+
+
+def test_rcrit_infinite_is_the_unsplit_walk_and_small_rcrit_shortens_lists(oracle):
+    pos = W.nfw(6000, seed=3)
+    t = oracle.build_tree(pos)
+    eps = 2.0 ** -8
+    boot, _ = oracle.walk_tree(t, eps=eps, mac_kind=1, mac_param=0.5)
+    aold = np.linalg.norm(boot[:, :3], axis=1).astype(np.float32)
+    kw = dict(eps=eps, mac_kind=0, mac_param=2.0 ** -9, aold=aold)
+    a, ca = oracle.walk_tree(t, **kw)
+    b, cb = oracle.walk_tree(t, r_crit=float("inf"), **kw)
+    assert np.array_equal(a, b) and ca == cb
+    s, cs = oracle.walk_tree(t, r_crit=0.25, **kw)
+    assert cs["groups"] > ca["groups"] and cs["interactions"] < ca["interactions"]   # tighter balls => shorter lists (P:122)
+    direct = oracle.direct(t.pos_sorted, eps)
+    err = lambda o: np.median(np.linalg.norm(o[:, :3] - direct[:, :3], axis=1) / np.linalg.norm(direct[:, :3], axis=1))
+    # a tight ball accepts cells right at the eq. 5 threshold, a wide one opens more than it must: the error moves towards
+    # (never far beyond) the per-particle criterion's Delta_acc-sized error
+    assert err(a) <= err(s) < 2.0 * 2.0 ** -9
+
+
+def test_rcrit_zero_is_the_textbook_per_particle_tree_walk(oracle):
+    """r_crit = 0: every particle walks alone with b_I = 0, i.e. the classic Barnes-Hut walk with the point MAC of eq. 5
+    (d = |r_J - r_i|).  Pure-Python recursive restatement on a tiny case, fp32 MAC arithmetic, double sums."""
+    n = 400
+    pos = W.plummer(n, seed=12)
+    t = oracle.build_tree(pos, n_leaf=4)
+    eps, dacc = 0.02, 2.0 ** -6
+    boot = oracle.direct(t.pos_sorted, eps)
+    aold = np.linalg.norm(boot[:, :3], axis=1).astype(np.float32)
+    out, c = oracle.walk_tree(t, eps=eps, mac_kind=0, mac_param=dacc, aold=aold, r_crit=0.0)
+    f32, P = np.float32, t.pos_sorted
+    eps2 = float(f32(eps)) ** 2
+    ref = np.zeros((n, 4))
+    n_int = 0
+    for i in range(n):
+        thr = f32(dacc) * aold[i]
+        stack = [0]
+        while stack:
+            J = stack.pop()
+            d3 = (t.com[J, :3] - P[i, :3]).astype(f32)
+            r2 = f32(np.float64(d3[2]) ** 2 + f32(np.float64(d3[1]) ** 2 + f32(d3[0] * d3[0])))   # fmaf = one rounding of the exact product-sum
+            d = f32(np.sqrt(r2))
+            mb2 = f32(f32(t.com[J, 3] * t.b[J]) * t.b[J])
+            if d > 0 and f32(thr * f32(f32(d * d) * f32(d * d))) >= mb2:
+                src = [(t.com[J].astype(np.float64))]
+            elif t.child[J] == 0xFFFFFFFF:
+                src = [P[s].astype(np.float64) for s in range(t.head[J], t.head[J] + t.num[J]) if s != i]
+                n_int += 1 if t.head[J] <= i < t.head[J] + t.num[J] else 0   # the walk counts the self entry (P:331 convention)
+            else:
+                stack.extend(range(t.child[J], t.child[J] + t.nchild[J]))
+                continue
+            for q in src:
+                dx = q[:3] - P[i, :3].astype(np.float64)
+                u = 1.0 / np.sqrt(dx @ dx + eps2)
+                ref[i, :3] += q[3] * u ** 3 * dx
+                ref[i, 3] -= q[3] * u
+                n_int += 1
+    assert c["groups"] == n and c["interactions"] == n_int
+    assert np.allclose(out, ref, rtol=1e-11, atol=1e-13)
