@@ -113,6 +113,7 @@ def run_reference(args, rank: int, world: int):
     t0 = time.time()
     pos, cfg = W.make_config(args.workload, seed=args.seed, n=args.n)
     n, eps, dacc = cfg["n"], cfg["eps"], cfg["delta_acc"]
+    r_crit = cfg["r_crit"] if args.r_crit is None else args.r_crit
     t_gen = time.time() - t0
     t0 = time.time()
     tree = oracle.build_tree(pos)
@@ -130,7 +131,7 @@ def run_reference(args, rank: int, world: int):
     def step():
         cnt = 0
         for lo, hi in ranges:
-            _, c = oracle.walk_tree(tree, eps=eps, mac_kind=0, mac_param=dacc, aold=aold, group_range=(lo, hi))
+            _, c = oracle.walk_tree(tree, eps=eps, mac_kind=0, mac_param=dacc, aold=aold, group_range=(lo, hi), r_crit=r_crit)
             cnt += c["interactions"]
         return cnt
 
@@ -146,7 +147,7 @@ def run_reference(args, rank: int, world: int):
               f"fp64 accumulation, {inter // args.steps} interactions per step; oracle tree build {t_build:.1f} s (untimed)")
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-            "data": "synthetic", "config": {"workload": args.workload, "n": n, "eps": eps, "delta_acc": dacc, "seed": args.seed},
+            "data": "synthetic", "config": {"workload": args.workload, "n": n, "eps": eps, "delta_acc": dacc, "r_crit": r_crit, "seed": args.seed},
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0, "setup_s": {"generate": t_gen, "oracle_build": t_build}}
@@ -166,7 +167,7 @@ def _sample_ranges(n_groups: int, want: int, pieces: int):
     return out
 
 
-def cpu_baseline(pos, cfg, budget_s: float = 15.0) -> dict:
+def cpu_baseline(pos, cfg, r_crit: float, budget_s: float = 15.0) -> dict:
     """Oracle walk (fp64 sum, OpenMP over groups) on a sample of the all-active substep sized to ~budget_s."""
     import oracle
     n, eps, dacc = cfg["n"], cfg["eps"], cfg["delta_acc"]
@@ -185,7 +186,7 @@ def cpu_baseline(pos, cfg, budget_s: float = 15.0) -> dict:
         t0 = time.time()
         cnt = 0
         for lo, hi in ranges:
-            _, c = oracle.walk_tree(tree, eps=eps, mac_kind=0, mac_param=dacc, aold=aold, group_range=(lo, hi))
+            _, c = oracle.walk_tree(tree, eps=eps, mac_kind=0, mac_param=dacc, aold=aold, group_range=(lo, hi), r_crit=r_crit)
             cnt += c["interactions"]
         return cnt, time.time() - t0
 
@@ -217,6 +218,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     pos_np, cfg = W.make_config(args.workload, seed=args.seed + rank, n=args.n)
     n, eps, dacc = cfg["n"], cfg["eps"], cfg["delta_acc"]
     block = cfg["block"]
+    r_crit = cfg["r_crit"] if args.r_crit is None else args.r_crit
     props = torch.cuda.get_device_properties(dev)
 
     g = Gothic(n)
@@ -232,8 +234,8 @@ def run_ours(args, rank: int, world: int, local_rank: int):
 
     # ---- untimed bootstrap (R7): opening-angle walk -> |a_old|, then one acceleration-MAC walk -------------
     g.build_tree(pos)
-    g.walk_tree(acc, eps=eps, mac_kind=MAC_OPENING_ANGLE, mac_param=THETA_BOOTSTRAP, amag_out=amag)
-    g.walk_tree(acc, eps=eps, mac_kind=MAC_ACCELERATION, mac_param=dacc, aold=amag, amag_out=amag)
+    g.walk_tree(acc, eps=eps, mac_kind=MAC_OPENING_ANGLE, mac_param=THETA_BOOTSTRAP, amag_out=amag, r_crit=r_crit)
+    g.walk_tree(acc, eps=eps, mac_kind=MAC_ACCELERATION, mac_param=dacc, aold=amag, amag_out=amag, r_crit=r_crit)
     if block:
         g.set_timesteps(level, acc_pot=acc, eps=eps, eta=ETA, max_levels=MAX_LEVELS, emin_nlev_dev=emin_nlev)
         g.check()
@@ -263,10 +265,10 @@ def run_ours(args, rank: int, world: int, local_rank: int):
                 timed("active", lambda: g.set_timesteps(level, acc_pot=None, eps=eps, substep=s, active=active, n_active_dev=n_act))
                 timed("moments", lambda: g.update_moments())
                 timed("walk", lambda: g.walk_tree(acc, eps=eps, mac_kind=MAC_ACCELERATION, mac_param=dacc, aold=amag, active=active,
-                                                   n_active_dev=n_act, amag_out=amag,
+                                                   n_active_dev=n_act, amag_out=amag, r_crit=r_crit,
                                                    n_interactions=None if counts is None else counts[s - 1:s]))
             else:
-                timed("walk", lambda: g.walk_tree(acc, eps=eps, mac_kind=MAC_ACCELERATION, mac_param=dacc, aold=amag, amag_out=amag,
+                timed("walk", lambda: g.walk_tree(acc, eps=eps, mac_kind=MAC_ACCELERATION, mac_param=dacc, aold=amag, amag_out=amag, r_crit=r_crit,
                                                    n_interactions=None if counts is None else counts[s - 1:s]))
 
     def barrier():
@@ -335,7 +337,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         h_out = torch.empty(n, 4, dtype=torch.float32).pin_memory()
         h_lev = torch.empty(n, dtype=torch.uint8).pin_memory()
         del acc_prev_orig, perm
-        g.block_cycle_host(pos_host, h_prev, h_out, eps=eps, delta_acc=dacc, eta=ETA, max_levels=MAX_LEVELS, level_host=h_lev)   # warm-up
+        g.block_cycle_host(pos_host, h_prev, h_out, eps=eps, delta_acc=dacc, eta=ETA, max_levels=MAX_LEVELS, level_host=h_lev, r_crit=r_crit)   # warm-up
         h_prev.copy_(h_prev0)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         barrier()
@@ -343,7 +345,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         e0.record()
         a, b = h_prev, h_out
         for _ in range(k_e2e):
-            g.block_cycle_host(pos_host, a, b, eps=eps, delta_acc=dacc, eta=ETA, max_levels=MAX_LEVELS, level_host=h_lev)
+            g.block_cycle_host(pos_host, a, b, eps=eps, delta_acc=dacc, eta=ETA, max_levels=MAX_LEVELS, level_host=h_lev, r_crit=r_crit)
             a, b = b, a
         e1.record()
         barrier()
@@ -353,7 +355,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         h_prev.copy_(h_prev0)
         a, b, e2e_inter = h_prev, h_out, 0
         for _ in range(k_e2e):
-            info = g.block_cycle_host(pos_host, a, b, eps=eps, delta_acc=dacc, eta=ETA, max_levels=MAX_LEVELS, level_host=h_lev, count=True)
+            info = g.block_cycle_host(pos_host, a, b, eps=eps, delta_acc=dacc, eta=ETA, max_levels=MAX_LEVELS, level_host=h_lev, count=True, r_crit=r_crit)
             e2e_inter += info["interactions"]
             a, b = b, a
         e2e = {"ms": e2e_ms, "steps": k_e2e, "interactions": e2e_inter, "h2d": 2 * n * 16, "d2h": n * 16 + n}
@@ -377,7 +379,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
             "ms_per_step": total_ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
-            "config": {"workload": args.workload, "n": n, "eps": eps, "delta_acc": dacc, "eta": ETA, "max_levels": MAX_LEVELS, "seed": args.seed,
+            "config": {"workload": args.workload, "n": n, "eps": eps, "delta_acc": dacc, "r_crit": r_crit, "eta": ETA, "max_levels": MAX_LEVELS, "seed": args.seed,
                        "group_size": 32, "n_leaf": 16, "key": "peano_hilbert", "n_levels": n_levels, "n_substeps": n_sub,
                        "parallelism": "replicas" if world > 1 else "single_gpu", "l2": "inputs_exceed_l2" if n * 16 > 126e6 else "inputs_fit_l2"},
             "sec_per_block_step": total_ms_max * 1e-3 / K / n_sub,
@@ -402,7 +404,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
                            "d2h_bytes_per_step": e2e["d2h"], "ms_per_step": e2e_ms_max / e2e["steps"], "steps": e2e["steps"]}
         if world == 1 and not args.no_cpu_baseline:
             del g
-            line["cpu_baseline"] = cpu_baseline(pos_np, cfg, args.cpu_budget)
+            line["cpu_baseline"] = cpu_baseline(pos_np, cfg, r_crit, args.cpu_budget)
         print(json.dumps(line), flush=True)
     if dist is not None:
         dist.barrier()
@@ -418,6 +420,7 @@ def main():
     ap.add_argument("--workload", default="nfw_2p24_block")
     ap.add_argument("--n", type=int, default=None, help="override N (debugging; the reported config then says so)")
     ap.add_argument("--seed", type=int, default=1)
+    ap.add_argument("--r-crit", type=float, default=None, help="override the workload's critical separation (PAPER.md:122-126); inf = no group splitting")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-budget", type=float, default=15.0)
     ap.add_argument("--ref-groups", type=int, default=65536, help="i-groups per step of the --impl reference sample")

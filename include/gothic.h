@@ -79,14 +79,19 @@ int gothic_update_moments(gothic_ctx *ctx, const float *pos_m_sorted, void *stre
  *   mac_kind      GOTHIC_MAC_ACCELERATION: accept J iff d >= (m_J b_J^2 / (mac_param |a_old|))^(1/4)  (eq. 5)
  *                 GOTHIC_MAC_OPENING_ANGLE: accept J iff b_J / d <= mac_param                         (eq. 2)
  *                 d measured from the surface of the group's enclosing ball (eq. 6-7).
+ *   r_crit        critical separation of PAPER.md:122-126 (R13): a group's member list (ascending) whose
+ *                 enclosing ball has b_I > r_crit is cut into its first ceil(k/2) members and the rest, recursively,
+ *                 until b_I <= r_crit or one member is left; every piece walks the tree on its own.  INFINITY = never
+ *                 split; 0 = every particle alone.  Must not be NaN or negative.  (The paper auto-tunes this number
+ *                 from timings; here it is the caller's.)
  *   aold          float[n] |a_old| per particle, sorted order; required iff mac_kind == ACCELERATION.
  *   acc_pot       float4[n] sorted order; ONLY active entries are written: (ax, ay, az, Phi).
  *   amag_out      optional float[n]: |a| of the new acceleration for active entries (may alias aold).
- *   n_interactions optional device counter, incremented by sum over groups (#members x list length)
+ *   n_interactions optional device counter, incremented by sum over walked pieces (#members x list length)
  *                 (counted in a separate run; pass NULL in timed runs).
  * Asynchronous. */
 int gothic_walk_tree(gothic_ctx *ctx, const uint32_t *active, uint32_t n_active, const uint32_t *n_active_dev,
-                     float eps, int mac_kind, float mac_param, const float *aold,
+                     float eps, int mac_kind, float mac_param, float r_crit, const float *aold,
                      float *acc_pot, float *amag_out, unsigned long long *n_interactions, void *stream);
 
 /* Block time steps (criterion from BASELINE.json configs[2], R6):
@@ -127,7 +132,7 @@ int gothic_check(gothic_ctx *ctx, void *stream);
  *   pos_m_host float4[n] HOST; aold_host float[n] HOST in ORIGINAL order (NULL allowed for opening-angle MAC);
  *   acc_pot_host float4[n] HOST out (sorted order); perm_host uint32[n] HOST out (may be NULL). */
 int gothic_gravity_host(gothic_ctx *ctx, const float *pos_m_host, uint32_t n, int key_kind, int n_leaf,
-                        float eps, int mac_kind, float mac_param, const float *aold_host,
+                        float eps, int mac_kind, float mac_param, float r_crit, const float *aold_host,
                         float *acc_pot_host, uint32_t *perm_host, void *stream);
 
 /* One full block-step cycle end to end with HOST buffers (bench.py "e2e"; the paper's per-step loop PAPER.md:179-187
@@ -143,7 +148,7 @@ int gothic_gravity_host(gothic_ctx *ctx, const float *pos_m_host, uint32_t n, in
  *   n_interactions_host  optional HOST out: interactions summed over the cycle (enables the device counter;
  *                        pass NULL in timed runs). */
 int gothic_block_cycle_host(gothic_ctx *ctx, const float *pos_m_host, const float *acc_prev_host, uint32_t n, int key_kind,
-                            int n_leaf, float eps, float eta, int max_levels, float delta_acc, float *acc_pot_host,
+                            int n_leaf, float eps, float eta, int max_levels, float delta_acc, float r_crit, float *acc_pot_host,
                             uint8_t *level_host, int32_t *info_host, unsigned long long *n_interactions_host, void *stream);
 
 /* Number of kernels this library has launched through this context (bench.py "gpu_launches"). */

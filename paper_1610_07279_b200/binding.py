@@ -61,7 +61,7 @@ def load_library():
     L.gothic_update_moments.restype = i32
     L.gothic_update_moments.argtypes = [vp, vp, vp]
     L.gothic_walk_tree.restype = i32
-    L.gothic_walk_tree.argtypes = [vp, vp, u32, vp, f32, i32, f32, vp, vp, vp, vp, vp]
+    L.gothic_walk_tree.argtypes = [vp, vp, u32, vp, f32, i32, f32, f32, vp, vp, vp, vp, vp]
     L.gothic_set_timesteps.restype = i32
     L.gothic_set_timesteps.argtypes = [vp, vp, u32, f32, f32, i32, u32, vp, vp, vp, vp, vp]
     L.gothic_get_tree_view.restype = i32
@@ -69,9 +69,9 @@ def load_library():
     L.gothic_check.restype = i32
     L.gothic_check.argtypes = [vp, vp]
     L.gothic_gravity_host.restype = i32
-    L.gothic_gravity_host.argtypes = [vp, vp, u32, i32, i32, f32, i32, f32, vp, vp, vp, vp]
+    L.gothic_gravity_host.argtypes = [vp, vp, u32, i32, i32, f32, i32, f32, f32, vp, vp, vp, vp]
     L.gothic_block_cycle_host.restype = i32
-    L.gothic_block_cycle_host.argtypes = [vp, vp, vp, u32, i32, i32, f32, f32, i32, f32, vp, vp, vp, vp, vp]
+    L.gothic_block_cycle_host.argtypes = [vp, vp, vp, u32, i32, i32, f32, f32, i32, f32, f32, vp, vp, vp, vp, vp]
     L.gothic_launch_count.restype = C.c_ulonglong
     L.gothic_launch_count.argtypes = [vp]
     _lib = L
@@ -148,12 +148,12 @@ class Gothic:
 
     def walk_tree(self, acc_pot: torch.Tensor, *, eps: float, mac_kind: int, mac_param: float, aold: torch.Tensor | None = None,
                   active: torch.Tensor | None = None, n_active: int | None = None, n_active_dev: torch.Tensor | None = None,
-                  amag_out: torch.Tensor | None = None, n_interactions: torch.Tensor | None = None):
+                  amag_out: torch.Tensor | None = None, n_interactions: torch.Tensor | None = None, r_crit: float = float("inf")):
         na = 0
         if active is not None:
             na = int(active.shape[0] if n_active is None else n_active)
         self._chk(self._L.gothic_walk_tree(self._ctx, _ptr(active, torch.int32) if active is not None else None, na,
-                                           _ptr(n_active_dev, torch.int32), float(eps), mac_kind, float(mac_param),
+                                           _ptr(n_active_dev, torch.int32), float(eps), mac_kind, float(mac_param), float(r_crit),
                                            _ptr(aold, torch.float32), _ptr(acc_pot, torch.float32), _ptr(amag_out, torch.float32),
                                            _ptr(n_interactions, torch.int64), _stream()))
 
@@ -188,18 +188,18 @@ class Gothic:
 
     def gravity_host(self, pos_m_host: torch.Tensor, acc_pot_host: torch.Tensor, *, eps: float, mac_kind: int, mac_param: float,
                      aold_host: torch.Tensor | None = None, perm_host: torch.Tensor | None = None,
-                     key_kind: int = KEY_PEANO_HILBERT, n_leaf: int = 16):
+                     key_kind: int = KEY_PEANO_HILBERT, n_leaf: int = 16, r_crit: float = float("inf")):
         """End to end with HOST (pinned) buffers: H2D, build, all-active walk, D2H."""
         for t in (pos_m_host, acc_pot_host, aold_host, perm_host):
             if t is not None and (t.is_cuda or not t.is_contiguous()):
                 raise GothicError("gravity_host expects contiguous host tensors")
         hp = lambda t: None if t is None else C.c_void_p(t.data_ptr())
         self._chk(self._L.gothic_gravity_host(self._ctx, hp(pos_m_host), pos_m_host.shape[0], key_kind, n_leaf, float(eps), mac_kind,
-                                              float(mac_param), hp(aold_host), hp(acc_pot_host), hp(perm_host), _stream()))
+                                              float(mac_param), float(r_crit), hp(aold_host), hp(acc_pot_host), hp(perm_host), _stream()))
 
     def block_cycle_host(self, pos_m_host: torch.Tensor, acc_prev_host: torch.Tensor, acc_pot_host: torch.Tensor, *, eps: float,
                          delta_acc: float, eta: float = 0.5, max_levels: int = 8, level_host: torch.Tensor | None = None,
-                         count: bool = False, key_kind: int = KEY_PEANO_HILBERT, n_leaf: int = 16) -> dict:
+                         count: bool = False, key_kind: int = KEY_PEANO_HILBERT, n_leaf: int = 16, r_crit: float = float("inf")) -> dict:
         """One full block-step cycle end to end with HOST (pinned) buffers: H2D, build, levels, all substeps, D2H."""
         for t in (pos_m_host, acc_prev_host, acc_pot_host, level_host):
             if t is not None and (t.is_cuda or not t.is_contiguous()):
@@ -208,6 +208,6 @@ class Gothic:
         info = (C.c_int32 * 4)()
         cnt = C.c_ulonglong(0)
         self._chk(self._L.gothic_block_cycle_host(self._ctx, hp(pos_m_host), hp(acc_prev_host), pos_m_host.shape[0], key_kind, n_leaf,
-                                                  float(eps), float(eta), max_levels, float(delta_acc), hp(acc_pot_host), hp(level_host),
+                                                  float(eps), float(eta), max_levels, float(delta_acc), float(r_crit), hp(acc_pot_host), hp(level_host),
                                                   C.cast(info, C.c_void_p), C.cast(C.pointer(cnt), C.c_void_p) if count else None, _stream()))
         return dict(e_min=info[0], n_levels=info[1], n_substeps=info[2], interactions=int(cnt.value) if count else None)

@@ -176,16 +176,16 @@ int gothic_update_moments(gothic_ctx *c, const float *pos_m_sorted, void *stream
 }
 
 int gothic_walk_tree(gothic_ctx *c, const uint32_t *active, uint32_t n_active, const uint32_t *n_active_dev,
-                     float eps, int mac_kind, float mac_param, const float *aold,
+                     float eps, int mac_kind, float mac_param, float r_crit, const float *aold,
                      float *acc_pot, float *amag_out, unsigned long long *n_interactions, void *stream)
 {
-    if (!c || !acc_pot || !(eps > 0.0f) || !(mac_param >= 0.0f)) return GOTHIC_ERR_ARG;
+    if (!c || !acc_pot || !(eps > 0.0f) || !(mac_param >= 0.0f) || !(r_crit >= 0.0f)) return GOTHIC_ERR_ARG;
     if (mac_kind != GOTHIC_MAC_ACCELERATION && mac_kind != GOTHIC_MAC_OPENING_ANGLE) return GOTHIC_ERR_ARG;
     if (mac_kind == GOTHIC_MAC_ACCELERATION && !aold) return GOTHIC_ERR_ARG;
     if (!c->built) return GOTHIC_ERR_STATE;
     if (active && !n_active_dev && n_active > c->n) return GOTHIC_ERR_ARG;
     if (active && !n_active_dev && n_active == 0) return GOTHIC_OK;
-    return gothic_stage_walk(c, active, n_active, n_active_dev, eps, mac_kind, mac_param, aold,
+    return gothic_stage_walk(c, active, n_active, n_active_dev, eps, mac_kind, mac_param, r_crit, aold,
                              reinterpret_cast<float4 *>(acc_pot), amag_out, n_interactions, static_cast<cudaStream_t>(stream));
 }
 
@@ -246,7 +246,7 @@ int gothic_get_tree_view(gothic_ctx *c, gothic_tree_view *out, void *stream)
 }
 
 int gothic_gravity_host(gothic_ctx *c, const float *pos_m_host, uint32_t n, int key_kind, int n_leaf,
-                        float eps, int mac_kind, float mac_param, const float *aold_host,
+                        float eps, int mac_kind, float mac_param, float r_crit, const float *aold_host,
                         float *acc_pot_host, uint32_t *perm_host, void *stream)
 {
     if (!c || !pos_m_host || !acc_pot_host || n == 0 || n > c->n_max) return GOTHIC_ERR_ARG;
@@ -268,7 +268,7 @@ int gothic_gravity_host(gothic_ctx *c, const float *pos_m_host, uint32_t n, int 
         k_gather_f32<<<(n + 255u) / 256u, 256, 0, s>>>(c->h2d_aold, c->idx[c->cur], n, c->d_aold_sorted);
         GOTHIC_LAUNCH_OK(c);
     }
-    rc = gothic_walk_tree(c, nullptr, 0, nullptr, eps, mac_kind, mac_param, aold_host ? c->d_aold_sorted : nullptr,
+    rc = gothic_walk_tree(c, nullptr, 0, nullptr, eps, mac_kind, mac_param, r_crit, aold_host ? c->d_aold_sorted : nullptr,
                           reinterpret_cast<float *>(c->d_acc), nullptr, nullptr, stream);
     if (rc != GOTHIC_OK) return rc;
     GOTHIC_CUDA_OK(c, cudaMemcpyAsync(acc_pot_host, c->d_acc, (size_t)n * sizeof(float4), cudaMemcpyDeviceToHost, s));
@@ -278,7 +278,7 @@ int gothic_gravity_host(gothic_ctx *c, const float *pos_m_host, uint32_t n, int 
 }
 
 int gothic_block_cycle_host(gothic_ctx *c, const float *pos_m_host, const float *acc_prev_host, uint32_t n, int key_kind, int n_leaf,
-                            float eps, float eta, int max_levels, float delta_acc, float *acc_pot_host, uint8_t *level_host,
+                            float eps, float eta, int max_levels, float delta_acc, float r_crit, float *acc_pot_host, uint8_t *level_host,
                             int32_t *info_host, unsigned long long *n_interactions_host, void *stream)
 {
     if (!c || !pos_m_host || !acc_prev_host || !acc_pot_host || n == 0 || n > c->n_max) return GOTHIC_ERR_ARG;
@@ -324,7 +324,7 @@ int gothic_block_cycle_host(gothic_ctx *c, const float *pos_m_host, const float 
         if (rc != GOTHIC_OK) return rc;
         rc = gothic_update_moments(c, nullptr, stream);   // the paper recomputes the pseudo j-particles every step
         if (rc != GOTHIC_OK) return rc;
-        rc = gothic_walk_tree(c, c->d_active, 0, n_active_dev, eps, GOTHIC_MAC_ACCELERATION, delta_acc, amag,
+        rc = gothic_walk_tree(c, c->d_active, 0, n_active_dev, eps, GOTHIC_MAC_ACCELERATION, delta_acc, r_crit, amag,
                               reinterpret_cast<float *>(c->d_acc), amag, n_interactions_host ? c->d_count : nullptr, stream);
         if (rc != GOTHIC_OK) return rc;
     }

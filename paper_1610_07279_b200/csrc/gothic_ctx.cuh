@@ -92,7 +92,7 @@ int gothic_stage_gather(gothic_ctx *c, const float4 *pos_m, uint32_t n, cudaStre
 int gothic_stage_nodes(gothic_ctx *c, uint32_t n, int n_leaf, cudaStream_t s);
 int gothic_stage_moments(gothic_ctx *c, cudaStream_t s);
 int gothic_stage_walk(gothic_ctx *c, const uint32_t *active, uint32_t n_active, const uint32_t *n_active_dev,
-                      float eps, int mac_kind, float mac_param, const float *aold, float4 *acc_pot,
+                      float eps, int mac_kind, float mac_param, float r_crit, const float *aold, float4 *acc_pot,
                       float *amag_out, unsigned long long *n_inter, cudaStream_t s);
 int gothic_stage_timesteps(gothic_ctx *c, const float4 *acc_pot, uint32_t n, float cconst, int max_levels,
                            uint32_t substep, uint8_t *level, uint32_t *active, uint32_t *n_active_dev,

@@ -30,13 +30,13 @@ def gpu_build(pos_m: np.ndarray, key_kind=0, n_leaf=16, group_size=32, node_max=
     return g, view_to_numpy(g.get_tree_view())
 
 
-def gpu_walk(g, n, *, eps, mac_kind, mac_param, aold=None, active=None, count=True, amag=False, n_active_dev=None):
+def gpu_walk(g, n, *, eps, mac_kind, mac_param, aold=None, active=None, count=True, amag=False, n_active_dev=None, r_crit=float("inf")):
     acc = torch.zeros(n, 4, dtype=torch.float32, device="cuda")
     cnt = torch.zeros(1, dtype=torch.int64, device="cuda") if count else None
     am = torch.zeros(n, dtype=torch.float32, device="cuda") if amag else None
     act = None if active is None else dev(active.astype(np.uint32), torch.int32)
     g.walk_tree(acc, eps=eps, mac_kind=mac_kind, mac_param=mac_param, aold=None if aold is None else dev(aold.astype(np.float32)),
-                active=act, n_active_dev=n_active_dev, amag_out=am, n_interactions=cnt)
+                active=act, n_active_dev=n_active_dev, amag_out=am, n_interactions=cnt, r_crit=r_crit)
     g.check()
     res = acc.cpu().numpy().astype(np.float64)
     return res, (int(cnt.item()) if count else None), (am.cpu().numpy() if amag else None)

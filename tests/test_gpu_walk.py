@@ -77,6 +77,40 @@ def test_walk_sparse_active_sets(oracle, frac, G):
     g.close()
 
 
+@pytest.mark.parametrize("r_crit,G,frac", [(0.0, 32, 1.0), (0.05, 32, 1.0), (0.3, 32, 0.6), (1.0, 32, 0.05), (0.2, 16, 1.0), (0.1, 8, 0.3)])
+def test_walk_rcrit_group_splitting(oracle, r_crit, G, frac):
+    """PAPER.md:122-126 / DESIGN.md R13: groups wider than r_crit are halved recursively; the pieces, their MAC decisions and
+    therefore the interaction counts must equal the oracle's exactly."""
+    from gpu_util import gpu_build, gpu_walk
+    n = 30011
+    pos = W.nfw(n, seed=6)
+    eps = 2.0 ** -8
+    g, v = gpu_build(pos, group_size=G)
+    aold = _bootstrap_aold(g, n, eps)
+    active = None if frac == 1.0 else W.random_active_subset(n, frac, seed=5)
+    rows = np.arange(n) if active is None else active
+    for kind, param in ((0, 2.0 ** -9), (1, 0.7)):
+        out, cnt, _ = gpu_walk(g, n, eps=eps, mac_kind=kind, mac_param=param, aold=aold, active=active, r_crit=r_crit)
+        ref, c = _oracle_on_gpu_tree(oracle, v, eps=eps, mac_kind=kind, mac_param=param, aold=aold, active=active, group_size=G, r_crit=r_crit)
+        assert cnt == c["interactions"]
+        _assert_parity(out, ref, rows)
+    if r_crit == 0.0:   # every particle alone: shorter lists than the unsplit walk
+        _, cnt_inf, _ = gpu_walk(g, n, eps=eps, mac_kind=1, mac_param=0.7, aold=aold, active=active)
+        assert cnt < cnt_inf
+    g.close()
+
+
+def test_walk_rejects_bad_rcrit():
+    from gpu_util import gpu_build
+    from paper_1610_07279_b200.binding import GothicError
+    g, v = gpu_build(W.plummer(100, seed=1))
+    acc = torch.zeros(100, 4, device="cuda")
+    for bad in (-1.0, float("nan")):
+        with pytest.raises(GothicError):
+            g.walk_tree(acc, eps=0.1, mac_kind=1, mac_param=0.5, r_crit=bad)
+    g.close()
+
+
 def test_walk_with_nothing_accepted_equals_direct_sum(oracle):
     """Delta_acc = 0: the walk degenerates to eq. 1; fp32 accumulation => 1e-5."""
     from gpu_util import gpu_build, gpu_walk, acc_rel_err
