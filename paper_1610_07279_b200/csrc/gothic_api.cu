@@ -14,9 +14,9 @@ cudaError_t dev_alloc(T **p, size_t count)
 
 void free_all(gothic_ctx *c)
 {
-    void *ptrs[] = {c->key[0], c->key[1], c->idx[0], c->idx[1], c->pos_sorted, c->box, c->bbox_bits,
+    void *ptrs[] = {c->key[0], c->key[1], c->idx[0], c->idx[1], c->items, c->box, c->bbox_bits,
                     c->node_head, c->node_num, c->node_child, c->node_parent, c->node_end, c->node_last,
-                    c->node_level, c->node_nchild, c->node_com, c->node_msum, c->node_b, c->node_b2bits, c->node_rec,
+                    c->node_level, c->node_nchild, c->node_com, c->node_msum, c->node_b, c->node_b2bits,
                     c->level_ofs, c->level_cnt, c->blk_cnt, c->flags, c->sort_tmp, c->grp_mask, c->grp_list, c->grp_cnt,
                     c->stack, c->ts_tmp, c->scan_tmp, c->h2d_pos, c->h2d_aold, c->d_aold_sorted, c->d_acc,
                     c->h2d_acc, c->d_level, c->d_active, c->d_cycle_info, c->d_count};
@@ -96,7 +96,7 @@ int gothic_create(gothic_ctx **out, uint32_t n_max, uint32_t node_max, int group
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device);
     if (e != cudaSuccess) { c->last_err = e; delete c; *out = nullptr; return GOTHIC_ERR_CUDA; }
     gothic_walk_config(c);
-    c->stack_cap = 4096;
+    c->stack_cap = 8192;   // u32 words of global spill area per resident warp (4096 families)
     if (scratch_bytes) {
         const size_t per = scratch_bytes / ((size_t)c->walk_warps * sizeof(uint32_t));
         if (per < 512) { delete c; *out = nullptr; return GOTHIC_ERR_ARG; }
@@ -109,13 +109,13 @@ int gothic_create(gothic_ctx **out, uint32_t n_max, uint32_t node_max, int group
 #define A(expr) if (e == cudaSuccess) e = (expr)
     A(dev_alloc(&c->key[0], n)); A(dev_alloc(&c->key[1], n));
     A(dev_alloc(&c->idx[0], n)); A(dev_alloc(&c->idx[1], n));
-    A(dev_alloc(&c->pos_sorted, n));
+    A(dev_alloc(&c->items, n + 2 * m));   // sorted particles, then the node records (walk.cu: one item space)
     A(dev_alloc(&c->box, 8)); A(dev_alloc(&c->bbox_bits, 8));
     A(dev_alloc(&c->node_head, m)); A(dev_alloc(&c->node_num, m)); A(dev_alloc(&c->node_child, m));
     A(dev_alloc(&c->node_parent, m)); A(dev_alloc(&c->node_end, m)); A(dev_alloc(&c->node_last, m));
     A(dev_alloc(&c->node_level, m)); A(dev_alloc(&c->node_nchild, m));
     A(dev_alloc(&c->node_com, m)); A(dev_alloc(&c->node_msum, m)); A(dev_alloc(&c->node_b, m));
-    A(dev_alloc(&c->node_b2bits, m)); A(dev_alloc(&c->node_rec, m));
+    A(dev_alloc(&c->node_b2bits, m));
     A(dev_alloc(&c->level_ofs, GOTHIC_NLEVP1 + 2)); A(dev_alloc(&c->level_cnt, GOTHIC_NLEVP1 + 2));
     A(dev_alloc(&c->blk_cnt, (size_t)2 * GOTHIC_NLEVP1 * c->nblk_max));
     A(dev_alloc(&c->flags, 4));
@@ -125,6 +125,10 @@ int gothic_create(gothic_ctx **out, uint32_t n_max, uint32_t node_max, int group
     A(dev_alloc(&c->ts_tmp, 4)); A(dev_alloc(&c->scan_tmp, (n + 2047) / 2048 + 1));
     A(cudaMemset(c->flags, 0, 4 * sizeof(uint32_t)));
 #undef A
+    if (e == cudaSuccess) {
+        c->pos_sorted = c->items;
+        c->node_rec = reinterpret_cast<NodeRec *>(c->items + n);
+    }
     if (e != cudaSuccess) {
         c->last_err = e;
         free_all(c);

@@ -10,13 +10,15 @@
 #define GOTHIC_LEAF 0xFFFFFFFFu
 #define GOTHIC_MAX_NLEAF 64
 
-// 32-byte node record read by the walk: one sector per MAC test.
+// 32-byte node record read by the walk: one sector per MAC test.  Sorted particles and node records share one
+// array of 16-byte items (particle s = item s, node J = items n_max + 2J and n_max + 2J + 1), and (w0, w1) is the
+// FAMILY the walk pushes when it opens the node: first item, count | particles << 31.
 struct __align__(16) NodeRec {
     float x, y, z, m;   // r_J, m_J
     float mb2;          // (m_J * b_J) * b_J   (eq. 5 right-hand side numerator, G = 1)
     float b;            // b_J
-    uint32_t w0;        // internal: first child id        | leaf: head (sorted index of first particle)
-    uint32_t w1;        // internal: number of children    | leaf: 0x80000000 | num
+    uint32_t w0;        // internal: item of the first child's record (n_max + 2 * child) | leaf: head (sorted index of first particle)
+    uint32_t w1;        // internal: number of children                                    | leaf: 0x80000000 | num
 };
 
 struct gothic_ctx {
@@ -37,7 +39,8 @@ struct gothic_ctx {
     uint64_t *key[2];      // double buffer for the sort
     uint32_t *idx[2];
     int cur;               // which half holds the sorted result
-    float4 *pos_sorted;
+    float4 *items;         // [n_max + 2 * node_max]: one allocation, item space of the walk
+    float4 *pos_sorted;    // = items
     float *box;            // [8]: xmin, ymin, zmin, side, scale, -, -, -
     uint32_t *bbox_bits;   // [6] ordered-int min/max accumulators
     // nodes
@@ -46,7 +49,7 @@ struct gothic_ctx {
     float4 *node_com, *node_msum;
     float *node_b;
     uint32_t *node_b2bits;
-    NodeRec *node_rec;
+    NodeRec *node_rec;     // = items + n_max
     uint32_t *level_ofs;   // [23]
     uint32_t *level_cnt;   // [22]
     uint32_t *blk_cnt;     // [2][22][nblk_max] per-block start/end event counts
@@ -59,8 +62,8 @@ struct gothic_ctx {
     uint32_t *grp_mask;    // [ceil(n_max/G)]
     uint32_t *grp_list;    // [ceil(n_max/G)]
     uint32_t *grp_cnt;     // [4]: 0 = number of non-empty groups, 1 = work counter
-    uint32_t *stack;       // per-warp traversal stacks
-    uint32_t stack_cap;    // entries per warp
+    uint32_t *stack;       // per-warp global spill areas of the traversal stacks
+    uint32_t stack_cap;    // u32 words per warp (2 per family)
     uint32_t walk_warps;   // resident warps of the persistent walk grid
     // time steps
     int32_t *ts_tmp;       // [4]: emin, lmax

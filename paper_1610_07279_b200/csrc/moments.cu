@@ -83,7 +83,7 @@ __global__ void __launch_bounds__(TPB) k_node_radius(uint32_t n_nodes, const flo
 __global__ void __launch_bounds__(TPB) k_pack_nodes(uint32_t n_nodes, const uint32_t *__restrict__ node_head, const uint32_t *__restrict__ node_num,
                                                      const uint32_t *__restrict__ node_child, const uint8_t *__restrict__ node_nchild,
                                                      const float4 *__restrict__ node_com, const uint32_t *__restrict__ node_b2bits,
-                                                     float *__restrict__ node_b, NodeRec *__restrict__ rec)
+                                                     float *__restrict__ node_b, NodeRec *__restrict__ rec, uint32_t root_item)
 {
     const uint32_t J = blockIdx.x * TPB + threadIdx.x;
     if (J >= n_nodes) return;
@@ -96,7 +96,7 @@ __global__ void __launch_bounds__(TPB) k_pack_nodes(uint32_t n_nodes, const uint
     r.b = b;
     const uint32_t c = node_child[J];
     if (c == GOTHIC_LEAF) { r.w0 = node_head[J]; r.w1 = 0x80000000u | node_num[J]; }
-    else { r.w0 = c; r.w1 = node_nchild[J]; }
+    else { r.w0 = root_item + 2u * c; r.w1 = node_nchild[J]; }
     rec[J] = r;
 }
 
@@ -116,7 +116,7 @@ int gothic_stage_moments(gothic_ctx *c, cudaStream_t s)
     }
     k_node_radius<<<grid, TPB, 0, s>>>(m, c->pos_sorted, c->node_head, c->node_num, c->node_child, c->node_parent, c->node_com, c->node_b2bits);
     GOTHIC_LAUNCH_OK(c);
-    k_pack_nodes<<<grid, TPB, 0, s>>>(m, c->node_head, c->node_num, c->node_child, c->node_nchild, c->node_com, c->node_b2bits, c->node_b, c->node_rec);
+    k_pack_nodes<<<grid, TPB, 0, s>>>(m, c->node_head, c->node_num, c->node_child, c->node_nchild, c->node_com, c->node_b2bits, c->node_b, c->node_rec, c->n_max);
     GOTHIC_LAUNCH_OK(c);
     return GOTHIC_OK;
 }
