@@ -103,9 +103,9 @@ __device__ __forceinline__ uint64_t spread3(uint32_t v)
     return w;
 }
 
-// B2: one thread per particle.  16 B in, 8 + 4 B out.
+// B2: one thread per particle.  16 B in, 8 B out.
 __global__ void __launch_bounds__(256) k_keys(const float4 *__restrict__ pos, uint32_t n, const float *__restrict__ box,
-                                              int key_kind, uint64_t *__restrict__ key, uint32_t *__restrict__ idx)
+                                              int key_kind, uint64_t *__restrict__ key)
 {
     const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
@@ -114,7 +114,6 @@ __global__ void __launch_bounds__(256) k_keys(const float4 *__restrict__ pos, ui
     const uint32_t ix = cell_coord(p.x, x0, scale), iy = cell_coord(p.y, y0, scale), iz = cell_coord(p.z, z0, scale);
     key[i] = key_kind == GOTHIC_KEY_PEANO_HILBERT ? peano_hilbert_63(ix, iy, iz)
                                                   : ((spread3(ix) << 2) | (spread3(iy) << 1) | spread3(iz));
-    idx[i] = i;
 }
 
 // B4: pos_sorted[s] = pos[perm[s]]
@@ -138,7 +137,7 @@ int gothic_stage_keys(gothic_ctx *c, const float4 *pos_m, uint32_t n, int key_ki
     k_box_finish<<<1, 1, 0, s>>>(c->bbox_bits, c->box);
     GOTHIC_LAUNCH_OK(c);
     c->cur = 0;
-    k_keys<<<(n + 255u) / 256u, 256, 0, s>>>(pos_m, n, c->box, key_kind, c->key[0], c->idx[0]);
+    k_keys<<<(n + 255u) / 256u, 256, 0, s>>>(pos_m, n, c->box, key_kind, c->key[0]);   // perm starts as the identity, generated by the first sort pass
     GOTHIC_LAUNCH_OK(c);
     return GOTHIC_OK;
 }

@@ -1,26 +1,224 @@
-// B3: stable LSD radix sort of (63-bit key, 32-bit index) pairs (the paper sorts with
-// cub::DeviceRadixSort::SortPairs).  Bring-up version: the CUB one-sweep sort that ships with the CUDA
-// toolkit, restricted to the 63 significant key bits; ties keep ascending original index (LSD radix is stable).
+// B3: stable LSD radix sort of (63-bit key, 32-bit index) pairs (the paper calls
+// cub::DeviceRadixSort::SortPairs).  Hand-written one-sweep sort for sm_100a:
+//
+//   k_sort_hist      one pass over the keys -> the 8 digit histograms (8 bits per digit, 63 significant bits),
+//   k_sort_scan      exclusive scan of each histogram = where every digit's run starts in the output of its pass,
+//   k_sort_onesweep  one launch per digit, least significant first.  A CTA takes the next tile of 4096 pairs (ticket
+//                    from an atomic counter, so that every earlier tile is already running), ranks its keys by
+//                    digit (warp-private counters + match.any, items in index order => stable), publishes its digit
+//                    counts, finds the sum over all earlier tiles by decoupled look-back (each of the 256 threads
+//                    chases one digit: aggregate -> inclusive flags in one 32-bit word with the count), regroups
+//                    keys and values by digit in shared memory and writes every run out contiguously.
+//
+// Per pass every pair is read once and written once (12 B each way): the HBM floor of an LSD radix sort.  Ties keep
+// ascending original index (LSD passes are stable), which is what makes perm bit-exact against the oracle's
+// std::stable_sort.
 #include "gothic_ctx.cuh"
-#include <cub/device/device_radix_sort.cuh>
+
+namespace {
+
+constexpr int RADIX = 256;
+constexpr int NPASS = 8;                    // 8 x 8 bits >= 63
+constexpr int SORT_TPB = 256;
+constexpr int SORT_WARPS = SORT_TPB / 32;
+constexpr int IPT = 16;                     // items per thread
+constexpr int TILE = SORT_TPB * IPT;        // 4096 pairs per CTA
+constexpr uint32_t ST_AGG = 1u << 30;       // status word: this tile's own count is in the low 30 bits
+constexpr uint32_t ST_INC = 1u << 31;       //              the count of this and ALL earlier tiles is
+constexpr uint32_t ST_VAL = ST_AGG - 1u;
+constexpr uint32_t FULL = 0xffffffffu;
+
+// scratch layout (u32 words): ghist[NPASS][RADIX] | ticket[NPASS] (+ pad to 16) | status[NPASS][ntiles][RADIX]
+__host__ __device__ inline size_t sort_words_head() { return (size_t)NPASS * RADIX + 16; }
+
+__global__ void __launch_bounds__(SORT_TPB) k_sort_hist(const uint64_t *__restrict__ key, uint32_t n, uint32_t *__restrict__ ghist)
+{
+    __shared__ uint32_t s_h[NPASS][RADIX];
+    for (int i = threadIdx.x; i < NPASS * RADIX; i += SORT_TPB) (&s_h[0][0])[i] = 0u;
+    __syncthreads();
+    const uint32_t stride = gridDim.x * SORT_TPB;
+    for (uint32_t i = blockIdx.x * SORT_TPB + threadIdx.x; i < n; i += stride) {
+        const uint64_t k = __ldg(key + i);
+#pragma unroll
+        for (int p = 0; p < NPASS; p++) atomicAdd(&s_h[p][(uint32_t)(k >> (8 * p)) & 255u], 1u);
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < NPASS * RADIX; i += SORT_TPB) {
+        const uint32_t v = (&s_h[0][0])[i];
+        if (v) atomicAdd(ghist + i, v);
+    }
+}
+
+// one CTA per pass: ghist[p][d] <- number of keys whose digit p is smaller than d
+__global__ void __launch_bounds__(RADIX) k_sort_scan(uint32_t *__restrict__ ghist)
+{
+    __shared__ uint32_t s_w[RADIX / 32];
+    uint32_t *h = ghist + blockIdx.x * RADIX;
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    const uint32_t v = h[threadIdx.x];
+    uint32_t incl = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t y = __shfl_up_sync(FULL, incl, o);
+        if (lane >= (uint32_t)o) incl += y;
+    }
+    if (lane == 31) s_w[warp] = incl;
+    __syncthreads();
+    uint32_t base = 0;
+    for (uint32_t w = 0; w < warp; w++) base += s_w[w];
+    h[threadIdx.x] = base + incl - v;
+}
+
+struct SortSmem {
+    uint64_t keys[TILE];                    // the tile regrouped by digit
+    uint32_t vals[TILE];
+    uint32_t hist[SORT_WARPS][RADIX];       // per-warp digit counters, then exclusive offsets across the warps
+    uint32_t dstart[RADIX];                 // where each digit's run starts inside the regrouped tile
+    uint32_t gbase[RADIX];                  // global position of slot j of digit d = gbase[d] + j
+    uint32_t wsum[SORT_WARPS];
+    uint32_t tile;
+};
+
+__global__ void __launch_bounds__(SORT_TPB) k_sort_onesweep(const uint64_t *__restrict__ kin, const uint32_t *__restrict__ vin,
+                                                            uint64_t *__restrict__ kout, uint32_t *__restrict__ vout, uint32_t n, int shift,
+                                                            const uint32_t *__restrict__ gstart, uint32_t *__restrict__ ticket,
+                                                            volatile uint32_t *status)
+{
+    extern __shared__ __align__(16) unsigned char s_raw[];
+    SortSmem &S = *reinterpret_cast<SortSmem *>(s_raw);
+    const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;
+    const uint32_t lt = (1u << lane) - 1u;
+
+    if (tid == 0) S.tile = atomicAdd(ticket, 1u);
+    for (int i = tid; i < SORT_WARPS * RADIX; i += SORT_TPB) (&S.hist[0][0])[i] = 0u;
+    __syncthreads();
+    const uint32_t tile = S.tile;
+    const uint32_t base = tile * (uint32_t)TILE;
+    const uint32_t n_valid = min((uint32_t)TILE, n - base);
+
+    // ---- load: warp w owns the 512 consecutive pairs [512 w, 512 w + 512) of the tile, 32 at a time ----
+    uint64_t k[IPT];
+    uint32_t v[IPT];
+#pragma unroll
+    for (int i = 0; i < IPT; i++) {
+        const uint32_t j = warp * (32u * IPT) + (uint32_t)i * 32u + lane;
+        k[i] = j < n_valid ? __ldg(kin + base + j) : ~0ull;
+        v[i] = j < n_valid ? (vin ? __ldg(vin + base + j) : base + j) : 0u;
+    }
+    // ---- rank inside (warp, digit), in index order ----
+    uint32_t pos[IPT];
+#pragma unroll
+    for (int i = 0; i < IPT; i++) {
+        const uint32_t j = warp * (32u * IPT) + (uint32_t)i * 32u + lane;
+        const bool valid = j < n_valid;
+        const uint32_t d = (uint32_t)(k[i] >> shift) & 255u;
+        const uint32_t peers = __match_any_sync(FULL, valid ? d : 256u);
+        const int leader = __ffs(peers) - 1;
+        uint32_t old = 0;
+        if ((int)lane == leader && valid) { old = S.hist[warp][d]; S.hist[warp][d] = old + __popc(peers); }
+        old = __shfl_sync(FULL, old, leader);
+        pos[i] = old + __popc(peers & lt);
+        __syncwarp();
+    }
+    __syncthreads();
+
+    // ---- thread t = digit t: offsets across the warps, run starts inside the tile, look-back over earlier tiles ----
+    {
+        uint32_t count = 0;
+#pragma unroll
+        for (int w = 0; w < SORT_WARPS; w++) {
+            const uint32_t c = S.hist[w][tid];
+            S.hist[w][tid] = count;
+            count += c;
+        }
+        volatile uint32_t *st = status + (size_t)tile * RADIX + tid;
+        if (tile == 0) *st = count | ST_INC;
+        else *st = count | ST_AGG;
+        // exclusive scan of the counts over the digits
+        uint32_t incl = count;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t y = __shfl_up_sync(FULL, incl, o);
+            if (lane >= (uint32_t)o) incl += y;
+        }
+        if (lane == 31) S.wsum[warp] = incl;
+        __syncthreads();
+        uint32_t wbase = 0;
+        for (uint32_t w = 0; w < warp; w++) wbase += S.wsum[w];
+        const uint32_t excl = wbase + incl - count;
+        S.dstart[tid] = excl;
+        // decoupled look-back: sum of this digit's counts over tiles tile-1, tile-2, ... until an inclusive one
+        uint32_t prefix = 0;
+        if (tile > 0) {
+            uint32_t t = tile - 1;
+            for (;;) {
+                const uint32_t s = status[(size_t)t * RADIX + tid];
+                if (s & ST_INC) { prefix += s & ST_VAL; break; }
+                if (s & ST_AGG) { prefix += s & ST_VAL; t--; continue; }
+                __nanosleep(20);
+            }
+            *st = (prefix + count) | ST_INC;
+        }
+        S.gbase[tid] = gstart[tid] + prefix - excl;
+    }
+    __syncthreads();
+
+    // ---- regroup by digit in shared memory ----
+#pragma unroll
+    for (int i = 0; i < IPT; i++) {
+        const uint32_t j = warp * (32u * IPT) + (uint32_t)i * 32u + lane;
+        if (j < n_valid) {
+            const uint32_t d = (uint32_t)(k[i] >> shift) & 255u;
+            const uint32_t p = S.dstart[d] + S.hist[warp][d] + pos[i];
+            S.keys[p] = k[i];
+            S.vals[p] = v[i];
+        }
+    }
+    __syncthreads();
+    // ---- write every run out contiguously ----
+#pragma unroll
+    for (int i = 0; i < IPT; i++) {
+        const uint32_t j = tid + (uint32_t)i * SORT_TPB;
+        if (j < n_valid) {
+            const uint64_t key = S.keys[j];
+            const uint32_t dst = S.gbase[(uint32_t)(key >> shift) & 255u] + j;
+            kout[dst] = key;
+            vout[dst] = S.vals[j];
+        }
+    }
+}
+
+} // namespace
 
 size_t gothic_sort_scratch_bytes(uint32_t n_max)
 {
-    size_t bytes = 0;
-    cub::DoubleBuffer<uint64_t> k(nullptr, nullptr);
-    cub::DoubleBuffer<uint32_t> v(nullptr, nullptr);
-    cub::DeviceRadixSort::SortPairs(nullptr, bytes, k, v, (int)n_max, 0, 63);
-    return bytes + 256;
+    const size_t ntiles = ((size_t)n_max + TILE - 1) / TILE;
+    return (sort_words_head() + (size_t)NPASS * ntiles * RADIX) * sizeof(uint32_t);
 }
 
 int gothic_stage_sort(gothic_ctx *c, uint32_t n, cudaStream_t s)
 {
-    cub::DoubleBuffer<uint64_t> k(c->key[c->cur], c->key[c->cur ^ 1]);
-    cub::DoubleBuffer<uint32_t> v(c->idx[c->cur], c->idx[c->cur ^ 1]);
-    size_t bytes = c->sort_tmp_bytes;
-    GOTHIC_CUDA_OK(c, cub::DeviceRadixSort::SortPairs(c->sort_tmp, bytes, k, v, (int)n, 0, 63, s));
-    c->launches += 9; // histogram + 8 one-sweep digit passes
-    c->cur = (k.Current() == c->key[0]) ? 0 : 1;
-    if (v.Current() != c->idx[c->cur]) return GOTHIC_ERR_CUDA;
+    static bool configured = false;
+    if (!configured) {
+        cudaFuncSetAttribute(k_sort_onesweep, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem));
+        configured = true;
+    }
+    const uint32_t ntiles = (n + TILE - 1) / TILE;
+    uint32_t *words = static_cast<uint32_t *>(c->sort_tmp);
+    uint32_t *ghist = words, *ticket = words + NPASS * RADIX, *status = words + sort_words_head();
+    GOTHIC_CUDA_OK(c, cudaMemsetAsync(words, 0, (sort_words_head() + (size_t)NPASS * ntiles * RADIX) * sizeof(uint32_t), s));
+    int grid = (int)((n + SORT_TPB - 1) / SORT_TPB);
+    if (grid > c->num_sms * 8) grid = c->num_sms * 8;
+    k_sort_hist<<<grid, SORT_TPB, 0, s>>>(c->key[c->cur], n, ghist);
+    GOTHIC_LAUNCH_OK(c);
+    k_sort_scan<<<NPASS, RADIX, 0, s>>>(ghist);
+    GOTHIC_LAUNCH_OK(c);
+    for (int p = 0; p < NPASS; p++) {
+        const int in = c->cur, out = c->cur ^ 1;
+        k_sort_onesweep<<<ntiles, SORT_TPB, sizeof(SortSmem), s>>>(c->key[in], p == 0 ? nullptr : c->idx[in], c->key[out], c->idx[out], n, 8 * p,
+                                                                    ghist + p * RADIX, ticket + p, status + (size_t)p * ntiles * RADIX);
+        GOTHIC_LAUNCH_OK(c);
+        c->cur = out;
+    }
     return GOTHIC_OK;
 }
