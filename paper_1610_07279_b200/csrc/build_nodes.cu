@@ -23,22 +23,58 @@ constexpr int NW = TPB / 32;
 
 struct Events { int s_lo, s_hi, e_lo, e_hi; };
 
-__device__ __forceinline__ Events node_events(const uint64_t *sk, int tid, uint32_t p, uint32_t n, int H)
+constexpr int KEYS_SM = TPB + 2 * GOTHIC_MAX_NLEAF;     // keys blockbase - H .. blockbase + TPB + H
+constexpr int WIN_SM = TPB + GOTHIC_MAX_NLEAF;          // window values of positions blockbase - H .. blockbase + TPB
+
+// D(p) is a sliding-window maximum of w(i) = shared_digits(key[i], key[i + H]) over i in [p - H, p]: every w is
+// computed once, then the window maxima of widths 2, 4, 8, ... are built by doubling in shared memory.
+// sw0 / sw1: ping-pong arrays of WIN_SM entries.  Returns D for the thread's own particle.
+__device__ __forceinline__ int window_depth(const uint64_t *sk, int8_t *sw0, int8_t *sw1, uint32_t n, int H)
 {
+    const long long g0 = (long long)blockIdx.x * TPB - H;          // particle index of window slot 0
+    const int len = TPB + H;
+    for (int t = threadIdx.x; t < len; t += TPB) {
+        const long long i = g0 + t;
+        sw0[t] = (i >= 0 && i + H < (long long)n) ? (int8_t)shared_digits(sk[t], sk[t + H]) : (int8_t)-1;
+    }
+    __syncthreads();
+    const int W = H + 1;                                            // window width
+    int8_t *cur = sw0, *nxt = sw1;
+    int k = 1;
+    while (2 * k <= W) {
+        for (int t = threadIdx.x; t + k < len; t += TPB) nxt[t] = max(cur[t], cur[t + k]);
+        for (int t = max(len - k, 0) + threadIdx.x; t < len; t += TPB) nxt[t] = cur[t];
+        __syncthreads();
+        int8_t *tmp = cur; cur = nxt; nxt = tmp;
+        k *= 2;
+    }
+    // cur[t] = max of w over slots [t, t + k); the thread's window is slots [tid, tid + W)
+    return max((int)cur[threadIdx.x], (int)cur[threadIdx.x + W - k]);
+}
+
+__device__ __forceinline__ Events node_events(const uint64_t *sk, int8_t *sw0, int8_t *sw1, int tid, uint32_t p, uint32_t n, int H)
+{
+    const int D = window_depth(sk, sw0, sw1, n, H);
     Events ev = {1, 0, 1, 0};
     if (p < n) {
         const uint64_t kp = sk[H + tid];
         const int dprev = p == 0 ? -1 : shared_digits(sk[H + tid - 1], kp);
         const int dnext = p == n - 1 ? -1 : shared_digits(kp, sk[H + tid + 1]);
-        int D = -1;
-        for (int w = 0; w <= H; w++) {
-            const long long i = (long long)p - H + w;
-            if (i >= 0 && i + H < (long long)n) D = max(D, shared_digits(sk[tid + w], sk[tid + w + H]));
-        }
         const int top = min(D + 1, GOTHIC_NLEV);
         ev.s_lo = dprev + 1; ev.s_hi = top; ev.e_lo = dnext + 1; ev.e_hi = top;
     }
     return ev;
+}
+
+// levels at which any lane of the warp has an event: [lo, hi] (empty if lo > hi)
+__device__ __forceinline__ void warp_level_range(const Events &ev, int &lo, int &hi)
+{
+    const bool any_s = ev.s_lo <= ev.s_hi, any_e = ev.e_lo <= ev.e_hi;
+    int l = GOTHIC_NLEVP1, h = -1;
+    if (any_s) { l = min(l, ev.s_lo); h = max(h, ev.s_hi); }
+    if (any_e) { l = min(l, ev.e_lo); h = max(h, ev.e_hi); }
+    lo = __reduce_min_sync(0xffffffffu, l);
+    hi = __reduce_max_sync(0xffffffffu, h);
 }
 
 __device__ __forceinline__ void load_keys(uint64_t *sk, const uint64_t *__restrict__ key, uint32_t n, int H)
@@ -55,13 +91,15 @@ __device__ __forceinline__ void load_keys(uint64_t *sk, const uint64_t *__restri
 __global__ void __launch_bounds__(TPB) k_count_events(const uint64_t *__restrict__ key, uint32_t n, int H,
                                                        uint32_t *__restrict__ blk_cnt, uint32_t nblk)
 {
-    __shared__ uint64_t sk[TPB + 2 * GOTHIC_MAX_NLEAF];
+    __shared__ uint64_t sk[KEYS_SM];
+    __shared__ int8_t sw[2][WIN_SM];
     __shared__ uint32_t tot[2][GOTHIC_NLEVP1];
     if (threadIdx.x < 2 * GOTHIC_NLEVP1) (&tot[0][0])[threadIdx.x] = 0;
     load_keys(sk, key, n, H);
-    const Events ev = node_events(sk, threadIdx.x, blockIdx.x * TPB + threadIdx.x, n, H);
-#pragma unroll
-    for (int L = 0; L < GOTHIC_NLEVP1; L++) {
+    const Events ev = node_events(sk, sw[0], sw[1], threadIdx.x, blockIdx.x * TPB + threadIdx.x, n, H);
+    int Llo, Lhi;
+    warp_level_range(ev, Llo, Lhi);
+    for (int L = Llo; L <= Lhi; L++) {
         const uint32_t bs = __ballot_sync(0xffffffffu, ev.s_lo <= L && L <= ev.s_hi);
         const uint32_t be = __ballot_sync(0xffffffffu, ev.e_lo <= L && L <= ev.e_hi);
         if (lane_id() == 0) {
@@ -75,17 +113,21 @@ __global__ void __launch_bounds__(TPB) k_count_events(const uint64_t *__restrict
 }
 
 // One block per (kind, level): exclusive scan over blocks in place; totals of the start rows -> level_cnt.
-__global__ void __launch_bounds__(TPB) k_scan_blocks(uint32_t *__restrict__ blk_cnt, uint32_t nblk, uint32_t *__restrict__ level_cnt)
+// 1024 threads x 8 consecutive counts per step.
+constexpr int SCAN_TPB = 1024, SCAN_IPT = 8;
+__global__ void __launch_bounds__(SCAN_TPB) k_scan_blocks(uint32_t *__restrict__ blk_cnt, uint32_t nblk, uint32_t *__restrict__ level_cnt)
 {
-    __shared__ uint32_t wsum[NW];
+    __shared__ uint32_t wsum[SCAN_TPB / 32];
     __shared__ uint32_t carry_s;
     uint32_t *row = blk_cnt + (size_t)blockIdx.x * nblk;
     if (threadIdx.x == 0) carry_s = 0;
     __syncthreads();
-    for (uint32_t b0 = 0; b0 < nblk; b0 += TPB) {
-        const uint32_t i = b0 + threadIdx.x;
-        const uint32_t v = i < nblk ? row[i] : 0u;
-        uint32_t x = v;
+    for (uint32_t b0 = 0; b0 < nblk; b0 += SCAN_TPB * SCAN_IPT) {
+        const uint32_t i0 = b0 + threadIdx.x * SCAN_IPT;
+        uint32_t v[SCAN_IPT], mine = 0;
+#pragma unroll
+        for (int k = 0; k < SCAN_IPT; k++) { v[k] = i0 + k < nblk ? row[i0 + k] : 0u; mine += v[k]; }
+        uint32_t x = mine;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
             const uint32_t y = __shfl_up_sync(0xffffffffu, x, o);
@@ -95,15 +137,16 @@ __global__ void __launch_bounds__(TPB) k_scan_blocks(uint32_t *__restrict__ blk_
         __syncthreads();
         uint32_t wpre = 0, total = 0;
 #pragma unroll
-        for (int w = 0; w < NW; w++) {
+        for (int w = 0; w < SCAN_TPB / 32; w++) {
             const uint32_t s = wsum[w];
             if (w < (int)(threadIdx.x >> 5)) wpre += s;
             total += s;
         }
-        const uint32_t carry = carry_s;
-        if (i < nblk) row[i] = carry + wpre + x - v;
+        uint32_t run = carry_s + wpre + x - mine;
+#pragma unroll
+        for (int k = 0; k < SCAN_IPT; k++) { if (i0 + k < nblk) row[i0 + k] = run; run += v[k]; }
         __syncthreads();
-        if (threadIdx.x == 0) carry_s = carry + total;
+        if (threadIdx.x == 0) carry_s += total;
         __syncthreads();
     }
     if (threadIdx.x == 0 && blockIdx.x < GOTHIC_NLEVP1) level_cnt[blockIdx.x] = carry_s;
@@ -129,15 +172,18 @@ __global__ void __launch_bounds__(TPB) k_emit_nodes(const uint64_t *__restrict__
                                                      uint32_t *__restrict__ node_child, uint32_t *__restrict__ node_end,
                                                      uint32_t *__restrict__ node_last)
 {
-    __shared__ uint64_t sk[TPB + 2 * GOTHIC_MAX_NLEAF];
+    __shared__ uint64_t sk[KEYS_SM];
+    __shared__ int8_t sw[2][WIN_SM];
     __shared__ uint32_t wcnt[2][GOTHIC_NLEVP1][NW];   // per-warp counts -> exclusive prefix + block base + level offset
     if (flags[0]) return;
+    for (int t = threadIdx.x; t < 2 * GOTHIC_NLEVP1 * NW; t += TPB) (&wcnt[0][0][0])[t] = 0u;
     load_keys(sk, key, n, H);
     const uint32_t p = blockIdx.x * TPB + threadIdx.x;
-    const Events ev = node_events(sk, threadIdx.x, p, n, H);
+    const Events ev = node_events(sk, sw[0], sw[1], threadIdx.x, p, n, H);
     const int warp = threadIdx.x >> 5;
-#pragma unroll
-    for (int L = 0; L < GOTHIC_NLEVP1; L++) {
+    int Llo, Lhi;
+    warp_level_range(ev, Llo, Lhi);
+    for (int L = Llo; L <= Lhi; L++) {
         const uint32_t bs = __ballot_sync(0xffffffffu, ev.s_lo <= L && L <= ev.s_hi);
         const uint32_t be = __ballot_sync(0xffffffffu, ev.e_lo <= L && L <= ev.e_hi);
         if (lane_id() == 0) { wcnt[0][L][warp] = __popc(bs); wcnt[1][L][warp] = __popc(be); }
@@ -152,8 +198,7 @@ __global__ void __launch_bounds__(TPB) k_emit_nodes(const uint64_t *__restrict__
     __syncthreads();
     const uint32_t lt = (1u << lane_id()) - 1u;
     uint32_t sid_below = GOTHIC_LEAF, eid_below = GOTHIC_LEAF;   // ids of this thread's events one level deeper
-#pragma unroll
-    for (int L = GOTHIC_NLEV; L >= 0; L--) {
+    for (int L = Lhi; L >= Llo; L--) {
         const bool fs = ev.s_lo <= L && L <= ev.s_hi, fe = ev.e_lo <= L && L <= ev.e_hi;
         const uint32_t bs = __ballot_sync(0xffffffffu, fs);
         const uint32_t be = __ballot_sync(0xffffffffu, fe);
@@ -200,7 +245,7 @@ int gothic_stage_nodes(gothic_ctx *c, uint32_t n, int n_leaf, cudaStream_t s)
     GOTHIC_CUDA_OK(c, cudaMemsetAsync(c->flags, 0, 4 * sizeof(uint32_t), s));
     k_count_events<<<nblk, TPB, 0, s>>>(key, n, n_leaf, c->blk_cnt, nblk);
     GOTHIC_LAUNCH_OK(c);
-    k_scan_blocks<<<2 * GOTHIC_NLEVP1, TPB, 0, s>>>(c->blk_cnt, nblk, c->level_cnt);
+    k_scan_blocks<<<2 * GOTHIC_NLEVP1, SCAN_TPB, 0, s>>>(c->blk_cnt, nblk, c->level_cnt);
     GOTHIC_LAUNCH_OK(c);
     k_level_offsets<<<1, 1, 0, s>>>(c->level_cnt, c->level_ofs, c->flags, c->node_max);
     GOTHIC_LAUNCH_OK(c);
