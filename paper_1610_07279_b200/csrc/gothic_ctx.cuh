@@ -47,6 +47,8 @@ struct gothic_ctx {
     uint32_t *node_head, *node_num, *node_child, *node_parent, *node_end, *node_last;
     uint8_t *node_level, *node_nchild;
     float4 *node_com, *node_msum;
+    float4 *node_up;       // (r_J, parent id as bits): one 16-byte load per level of the radius climb
+    uint32_t *leaf_of;     // [n_max] leaf node of every sorted particle
     float *node_b;
     uint32_t *node_b2bits;
     NodeRec *node_rec;     // = items + n_max

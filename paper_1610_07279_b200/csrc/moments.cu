@@ -4,34 +4,42 @@
 //
 // Mass and first moment go bottom-up (leaves from particles, internal nodes from their <= 8 contiguous
 // children, one launch per level from the deepest).  The radius needs every particle against every ancestor's
-// centre: one thread per leaf climbs the parent chain and raises b_J^2 with an integer atomicMax on the float
-// bits (non-negative floats order like unsigned ints), skipping the atomic when the stored value is already larger.
+// centre: one thread per PARTICLE (position in registers, read once) climbs from its leaf to the root; a level costs
+// one 16-byte load (r_J and the parent id share a record).  Consecutive sorted particles share their ancestors, so the
+// lanes of a warp form contiguous segments with the same node: the segment maximum is taken with shuffles (one
+// REDUX when the whole warp sits in one node, the usual case above the lowest levels) and only the first lane of a
+// segment raises b_J^2 with an integer atomicMax on the float bits (non-negative floats order like unsigned ints),
+// skipped when the stored value is already larger.
 #include "gothic_ctx.cuh"
 
 namespace {
 
 constexpr int TPB = 256;
 
-__device__ __forceinline__ void store_com(uint32_t J, float4 ms, float4 *__restrict__ node_msum, float4 *__restrict__ node_com,
-                                          uint32_t *__restrict__ node_b2bits)
+__device__ __forceinline__ void store_com(uint32_t J, float4 ms, float4 com, float4 *__restrict__ node_msum, float4 *__restrict__ node_com,
+                                          uint32_t *__restrict__ node_b2bits, const uint32_t *__restrict__ node_parent, float4 *__restrict__ node_up)
 {
     node_msum[J] = ms;
-    node_com[J] = make_float4(__fdiv_rn(ms.x, ms.w), __fdiv_rn(ms.y, ms.w), __fdiv_rn(ms.z, ms.w), ms.w);
+    node_com[J] = com;
     node_b2bits[J] = 0u;
+    node_up[J] = make_float4(com.x, com.y, com.z, __uint_as_float(node_parent[J]));
+}
+__device__ __forceinline__ float4 com_of(float4 ms)
+{
+    return make_float4(__fdiv_rn(ms.x, ms.w), __fdiv_rn(ms.y, ms.w), __fdiv_rn(ms.z, ms.w), ms.w);
 }
 
 __global__ void __launch_bounds__(TPB) k_leaf_moments(uint32_t n_nodes, const float4 *__restrict__ pos, const uint32_t *__restrict__ node_head,
                                                        const uint32_t *__restrict__ node_num, const uint32_t *__restrict__ node_child,
-                                                       float4 *__restrict__ node_msum, float4 *__restrict__ node_com, uint32_t *__restrict__ node_b2bits)
+                                                       float4 *__restrict__ node_msum, float4 *__restrict__ node_com, uint32_t *__restrict__ node_b2bits,
+                                                       const uint32_t *__restrict__ node_parent, float4 *__restrict__ node_up)
 {
     const uint32_t J = blockIdx.x * TPB + threadIdx.x;
     if (J >= n_nodes || node_child[J] != GOTHIC_LEAF) return;
     const uint32_t h = node_head[J], c = node_num[J];
     if (c == 1) {   // a single-particle node IS the particle (bitwise), b_J = 0
         const float4 p = __ldg(pos + h);
-        node_msum[J] = make_float4(p.w * p.x, p.w * p.y, p.w * p.z, p.w);
-        node_com[J] = p;
-        node_b2bits[J] = 0u;
+        store_com(J, make_float4(p.w * p.x, p.w * p.y, p.w * p.z, p.w), p, node_msum, node_com, node_b2bits, node_parent, node_up);
         return;
     }
     float4 ms = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -39,12 +47,13 @@ __global__ void __launch_bounds__(TPB) k_leaf_moments(uint32_t n_nodes, const fl
         const float4 p = __ldg(pos + j);
         ms.x = fmaf(p.w, p.x, ms.x); ms.y = fmaf(p.w, p.y, ms.y); ms.z = fmaf(p.w, p.z, ms.z); ms.w += p.w;
     }
-    store_com(J, ms, node_msum, node_com, node_b2bits);
+    store_com(J, ms, com_of(ms), node_msum, node_com, node_b2bits, node_parent, node_up);
 }
 
 __global__ void __launch_bounds__(TPB) k_internal_moments(uint32_t first, uint32_t count, const uint32_t *__restrict__ node_child,
                                                            const uint8_t *__restrict__ node_nchild, float4 *__restrict__ node_msum,
-                                                           float4 *__restrict__ node_com, uint32_t *__restrict__ node_b2bits)
+                                                           float4 *__restrict__ node_com, uint32_t *__restrict__ node_b2bits,
+                                                           const uint32_t *__restrict__ node_parent, float4 *__restrict__ node_up)
 {
     const uint32_t t = blockIdx.x * TPB + threadIdx.x;
     if (t >= count) return;
@@ -56,28 +65,95 @@ __global__ void __launch_bounds__(TPB) k_internal_moments(uint32_t first, uint32
         const float4 q = node_msum[c + k];
         ms.x += q.x; ms.y += q.y; ms.z += q.z; ms.w += q.w;
     }
-    store_com(J, ms, node_msum, node_com, node_b2bits);
+    store_com(J, ms, com_of(ms), node_msum, node_com, node_b2bits, node_parent, node_up);
 }
 
-__global__ void __launch_bounds__(TPB) k_node_radius(uint32_t n_nodes, const float4 *__restrict__ pos, const uint32_t *__restrict__ node_head,
-                                                      const uint32_t *__restrict__ node_num, const uint32_t *__restrict__ node_child,
-                                                      const uint32_t *__restrict__ node_parent, const float4 *__restrict__ node_com,
-                                                      uint32_t *__restrict__ node_b2bits)
+// Persistent warps, each sweeping a contiguous range of sorted particles 32 at a time.  Lane L of a warp remembers the
+// node the warp was last in at level L: id, particle range, centre and the running maximum.  While a chunk lies inside
+// the remembered range of a level, that level needs no memory access at all (centre broadcast by shuffle, one REDUX);
+// only the lowest levels, where the chunk straddles several nodes, climb parent links from the leaves.  A remembered
+// maximum is written out (guarded atomicMax) when the warp moves on to another node of that level or finishes, so the
+// upper levels, which every particle contributes to, cost a few thousand atomics in total.
+__global__ void __launch_bounds__(TPB) k_node_radius(uint32_t n, uint32_t per_warp, const float4 *__restrict__ pos,
+                                                      const uint32_t *__restrict__ leaf_of, const uint8_t *__restrict__ node_level,
+                                                      const uint32_t *__restrict__ node_head, const uint32_t *__restrict__ node_num,
+                                                      const float4 *__restrict__ node_up, uint32_t *__restrict__ node_b2bits)
 {
-    const uint32_t J = blockIdx.x * TPB + threadIdx.x;
-    if (J >= n_nodes || node_child[J] != GOTHIC_LEAF) return;
-    const uint32_t h = node_head[J], c = node_num[J];
-    for (uint32_t A = J; A != GOTHIC_LEAF; A = node_parent[A]) {
-        const float4 cm = node_com[A];
-        float d2max = 0.0f;
-        for (uint32_t j = h; j < h + c; j++) {
-            const float4 p = __ldg(pos + j);
-            const float dx = __fsub_rn(p.x, cm.x), dy = __fsub_rn(p.y, cm.y), dz = __fsub_rn(p.z, cm.z);
-            d2max = fmaxf(d2max, fmaf(dz, dz, fmaf(dy, dy, __fmul_rn(dx, dx))));
+    const uint32_t lane = lane_id();
+    const uint32_t gw = (blockIdx.x * TPB + threadIdx.x) >> 5;
+    const uint64_t r0 = (uint64_t)gw * per_warp;
+    if (r0 >= n) return;
+    const uint32_t r1 = (uint32_t)min((uint64_t)n, r0 + per_warp);
+    // lane L: level L
+    uint32_t m_node = GOTHIC_LEAF, m_head = 0u, m_end = 0u, m_max = 0u;
+    float m_x = 0.f, m_y = 0.f, m_z = 0.f;
+    // the next chunk's particle, leaf and leaf level are requested one chunk ahead
+    float4 p_nx = make_float4(0.f, 0.f, 0.f, 0.f);
+    uint32_t A_nx = GOTHIC_LEAF;
+    int lev_nx = -1;
+    if ((uint32_t)r0 + lane < r1) { p_nx = __ldg(pos + (uint32_t)r0 + lane); A_nx = __ldg(leaf_of + (uint32_t)r0 + lane); lev_nx = node_level[A_nx]; }
+    for (uint32_t s0 = (uint32_t)r0; s0 < r1; s0 += 32u) {
+        const uint32_t s = s0 + lane;
+        const bool act = s < r1;
+        const float4 p = p_nx;
+        uint32_t A = A_nx;
+        int lev = lev_nx;
+        p_nx = make_float4(0.f, 0.f, 0.f, 0.f); A_nx = GOTHIC_LEAF; lev_nx = -1;
+        if (s + 32u < r1) { p_nx = __ldg(pos + s + 32u); A_nx = __ldg(leaf_of + s + 32u); lev_nx = node_level[A_nx]; }
+        // ---- top-down over the levels whose remembered node contains the whole chunk (nested, so levels 0 .. Lf-1) ----
+        const uint32_t in_mask = __ballot_sync(0xffffffffu, m_node != GOTHIC_LEAF && s0 >= m_head && min(s0 + 32u, r1) <= m_end);
+        const int Lf = __ffs(~in_mask) - 1;
+        for (int L = 0; L < Lf; L++) {
+            const float cx = __shfl_sync(0xffffffffu, m_x, L), cy = __shfl_sync(0xffffffffu, m_y, L), cz = __shfl_sync(0xffffffffu, m_z, L);
+            const float dx = __fsub_rn(p.x, cx), dy = __fsub_rn(p.y, cy), dz = __fsub_rn(p.z, cz);
+            const uint32_t bits = act ? __float_as_uint(fmaf(dz, dz, fmaf(dy, dy, __fmul_rn(dx, dx)))) : 0u;
+            const uint32_t mx = __reduce_max_sync(0xffffffffu, bits);
+            if ((int)lane == L) m_max = max(m_max, mx);
         }
-        const uint32_t bits = __float_as_uint(d2max);
-        if (bits > *(volatile uint32_t *)(node_b2bits + A)) atomicMax(node_b2bits + A, bits);
+        // ---- bottom-up from the deepest leaf of the chunk to level Lf: a lane joins when the walk reaches its leaf's
+        //      level, so that the lanes that sit in the same node are neighbours; the record of the next level is
+        //      requested before the reduction of this one ----
+        int L = __reduce_max_sync(0xffffffffu, lev);
+        float4 u = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (lev == L && L >= Lf) u = node_up[A];
+        for (; L >= Lf; L--) {
+            const bool on = lev == L;
+            const uint32_t node = on ? A : GOTHIC_LEAF;
+            const float cx = u.x, cy = u.y, cz = u.z;
+            uint32_t bits = 0u;
+            if (on) {
+                const float dx = __fsub_rn(p.x, cx), dy = __fsub_rn(p.y, cy), dz = __fsub_rn(p.z, cz);
+                bits = __float_as_uint(fmaf(dz, dz, fmaf(dy, dy, __fmul_rn(dx, dx))));
+                A = __float_as_uint(u.w);
+                lev = L - 1;
+            }
+            if (lev == L - 1 && L > Lf) u = node_up[A];
+            int all_same = 0;
+            __match_all_sync(0xffffffffu, node, &all_same);
+            if (all_same) {                                                  // whole chunk in one node: remember it
+                bits = __reduce_max_sync(0xffffffffu, bits);
+                if ((int)lane == L) {
+                    if (m_node == node) m_max = max(m_max, bits);
+                    else {
+                        if (m_node != GOTHIC_LEAF && m_max > __ldcg(node_b2bits + m_node)) atomicMax(node_b2bits + m_node, m_max);
+                        m_node = node; m_max = bits;
+                        m_head = node_head[node]; m_end = m_head + node_num[node];
+                        m_x = cx; m_y = cy; m_z = cz;
+                    }
+                }
+            } else {                                                         // contiguous segments of equal node
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const uint32_t b2 = __shfl_down_sync(0xffffffffu, bits, o);
+                    const uint32_t n2 = __shfl_down_sync(0xffffffffu, node, o);
+                    if (lane + o < 32u && n2 == node) bits = max(bits, b2);
+                }
+                const uint32_t nprev = __shfl_up_sync(0xffffffffu, node, 1);
+                if (on && (lane == 0 || nprev != node)) atomicMax(node_b2bits + node, bits);      // low levels: distinct addresses, no guard
+            }
+        }
     }
+    if (m_node != GOTHIC_LEAF && m_max > __ldcg(node_b2bits + m_node)) atomicMax(node_b2bits + m_node, m_max);
 }
 
 __global__ void __launch_bounds__(TPB) k_pack_nodes(uint32_t n_nodes, const uint32_t *__restrict__ node_head, const uint32_t *__restrict__ node_num,
@@ -106,15 +182,22 @@ int gothic_stage_moments(gothic_ctx *c, cudaStream_t s)
 {
     const uint32_t m = c->n_nodes;
     const uint32_t grid = (m + TPB - 1) / TPB;
-    k_leaf_moments<<<grid, TPB, 0, s>>>(m, c->pos_sorted, c->node_head, c->node_num, c->node_child, c->node_msum, c->node_com, c->node_b2bits);
+    k_leaf_moments<<<grid, TPB, 0, s>>>(m, c->pos_sorted, c->node_head, c->node_num, c->node_child, c->node_msum, c->node_com, c->node_b2bits, c->node_parent, c->node_up);
     GOTHIC_LAUNCH_OK(c);
     for (int L = (int)c->n_levels_tree - 2; L >= 0; L--) {
         const uint32_t first = c->h_level_ofs[L], count = c->h_level_ofs[L + 1] - first;
         if (!count) continue;
-        k_internal_moments<<<(count + TPB - 1) / TPB, TPB, 0, s>>>(first, count, c->node_child, c->node_nchild, c->node_msum, c->node_com, c->node_b2bits);
+        k_internal_moments<<<(count + TPB - 1) / TPB, TPB, 0, s>>>(first, count, c->node_child, c->node_nchild, c->node_msum, c->node_com, c->node_b2bits, c->node_parent, c->node_up);
         GOTHIC_LAUNCH_OK(c);
     }
-    k_node_radius<<<grid, TPB, 0, s>>>(m, c->pos_sorted, c->node_head, c->node_num, c->node_child, c->node_parent, c->node_com, c->node_b2bits);
+    {
+        int per_sm = 0;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_node_radius, TPB, 0);
+        if (per_sm < 1) per_sm = 1;
+        const uint32_t blocks = (uint32_t)(c->num_sms * per_sm), warps = blocks * (TPB / 32);     // one resident wave
+        const uint32_t per_warp = (((c->n + warps - 1) / warps + 31u) / 32u) * 32u;
+        k_node_radius<<<blocks, TPB, 0, s>>>(c->n, per_warp, c->pos_sorted, c->leaf_of, c->node_level, c->node_head, c->node_num, c->node_up, c->node_b2bits);
+    }
     GOTHIC_LAUNCH_OK(c);
     k_pack_nodes<<<grid, TPB, 0, s>>>(m, c->node_head, c->node_num, c->node_child, c->node_nchild, c->node_com, c->node_b2bits, c->node_b, c->node_rec, c->n_max);
     GOTHIC_LAUNCH_OK(c);
