@@ -35,6 +35,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(OBJ, exist_ok=True)
     nvcc = os.environ.get("NVCC", "nvcc")
     extra = ["-Xptxas", "-v"] if verbose else []
+    extra += os.environ.get("GOTHIC_NVCC_EXTRA", "").split()      # e.g. -DGOTHIC_WALK_WARPS=7 (tuning knobs of walk.cu)
 
     def compile_one(src: str) -> str:
         obj = os.path.join(OBJ, src.replace(".cu", ".o"))
