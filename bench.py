@@ -41,6 +41,9 @@ METRIC = "tree_walk_interactions_per_s_block_cycle"
 UNIT = "interactions/s"
 FLOP_PER_INTERACTION = 24          # 20 + rsqrt counted as 4 (the paper's GTX TITAN X convention); 20 and 28 also reported
 THETA_BOOTSTRAP = 0.5              # DESIGN.md R7
+# dram__bytes_read.sum + dram__bytes_write.sum per k_walk launch, mean over the 8 substep launches of one cycle of the default
+# workload, from the ncu capture summarised in profiles/r01_walk_traffic.md (a profiler number: quoted, never measured here)
+NCU_WALK_TRAFFIC_BYTES = {"nfw_2p24_block": 344354880}
 ETA, MAX_LEVELS = 0.5, 8           # BASELINE.json configs[2]
 
 
@@ -391,7 +394,8 @@ def run_ours(args, rank: int, world: int, local_rank: int):
             "walk": {"interactions_per_s": walk_rate, "tflops_20": walk_rate * 20 / 1e12, "tflops_24": walk_rate * 24 / 1e12,
                      "tflops_28": walk_rate * 28 / 1e12, "frac_fp32_peak_24": achieved / alu_peak},
             "roofline": {"kernel": "k_walk", "bound": "alu", "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s", "frac": achieved / alu_peak,
-                         "traffic": None, "flop_per_interaction": FLOP_PER_INTERACTION,
+                         "traffic": NCU_WALK_TRAFFIC_BYTES.get(args.workload) if args.n is None else None, "traffic_unit": "bytes/launch",
+                         "flop_per_interaction": FLOP_PER_INTERACTION,
                          "avg_launch_ms": stage_ms["walk"] / max(walk_launches, 1),
                          "peak_source": f"derived: {props.multi_processor_count} SM x 128 FP32 lanes x 2 flop x {peaks['sm_max_mhz']:.0f} MHz "
                                         f"(clock from MEASURED_PEAKS.json, {peaks['source']})"},
