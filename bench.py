@@ -205,6 +205,18 @@ def cpu_baseline(pos, cfg, r_crit: float, budget_s: float = 15.0) -> dict:
 
 
 # ------------------------------------------------------------------------------------------------------------
+def aggregate_over_ranks(dist, times_ms, counts, device):
+    """Replicas only: no data-path collective.  The job's time is the MAX over ranks of each device time,
+    its work the SUM over ranks of each count.  `dist` is torch.distributed (any backend) or None for one rank."""
+    import torch
+    t_all = torch.tensor(list(times_ms), dtype=torch.float64, device=device)
+    i_all = torch.tensor(list(counts), dtype=torch.int64, device=device)
+    if dist is not None:
+        dist.all_reduce(t_all, op=dist.ReduceOp.MAX)
+        dist.all_reduce(i_all, op=dist.ReduceOp.SUM)
+    return [float(x) for x in t_all.tolist()], [int(x) for x in i_all.tolist()]
+
+
 def run_ours(args, rank: int, world: int, local_rank: int):
     import torch
     from paper_1610_07279_b200 import workloads as W
@@ -364,13 +376,8 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         e2e = {"ms": e2e_ms, "steps": k_e2e, "interactions": e2e_inter, "h2d": 2 * n * 16, "d2h": n * 16 + n}
 
     # ---- max over ranks, aggregate ---------------------------------------------------------------------------------------
-    t_all = torch.tensor([total_ms, stage_ms["walk"], e2e["ms"] if e2e else 0.0], dtype=torch.float64, device=dev)
-    i_all = torch.tensor([inter_total, e2e["interactions"] if e2e else 0], dtype=torch.int64, device=dev)
-    if dist is not None:
-        dist.all_reduce(t_all, op=dist.ReduceOp.MAX)
-        dist.all_reduce(i_all, op=dist.ReduceOp.SUM)
-    total_ms_max, walk_ms_max, e2e_ms_max = (float(x) for x in t_all.tolist())
-    inter_all, e2e_inter_all = (int(x) for x in i_all.tolist())
+    (total_ms_max, walk_ms_max, e2e_ms_max), (inter_all, e2e_inter_all) = aggregate_over_ranks(
+        dist, [total_ms, stage_ms["walk"], e2e["ms"] if e2e else 0.0], [inter_total, e2e["interactions"] if e2e else 0], dev)
 
     if rank == 0:
         K = args.steps
