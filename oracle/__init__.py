@@ -55,6 +55,11 @@ def lib():
         L.oracle_walk.argtypes = [_f32p, C.c_uint32, _u32p, _u32p, _u32p, _u8p, _f32p, _f32p,
                                   C.c_void_p, C.c_uint32, C.c_int, C.c_float, C.c_int, C.c_float, C.c_void_p,
                                   C.c_uint32, C.c_uint32, C.c_float, _f64p, _u64p]
+        L.oracle_predict.restype = None
+        L.oracle_predict.argtypes = [_f32p, _f32p, _f32p, _u32p, C.c_uint32, C.c_float, C.c_uint32, _f32p]
+        L.oracle_correct.restype = None
+        L.oracle_correct.argtypes = [_u32p, C.c_uint32, _f32p, _f32p, C.c_uint32, C.c_float, _f32p, _f32p, _f32p, _u32p,
+                                     C.c_void_p, C.c_float, C.c_int, C.c_int]
         L.oracle_group_ball.restype = None
         L.oracle_group_ball.argtypes = [_f32p, _u32p, C.c_uint32, _f32p]
         _lib = L
@@ -249,3 +254,28 @@ def group_ball(pos_sorted, members) -> np.ndarray:
     members = np.ascontiguousarray(members, np.uint32)
     lib().oracle_group_ball(_pos(pos_sorted), members, members.shape[0], out)
     return out
+
+
+def predict(pos_m, vel, acc_pot, t_last, t_now: int, dt_unit: float) -> np.ndarray:
+    """O8, eq. 15-16: all j-particles to t_now.  Returns pos_pred float32 [n,4]."""
+    pos_m = _pos(pos_m)
+    n = pos_m.shape[0]
+    out = np.zeros((n, 4), np.float32)
+    lib().oracle_predict(pos_m, np.ascontiguousarray(vel, np.float32), np.ascontiguousarray(acc_pot, np.float32),
+                         np.ascontiguousarray(t_last, np.uint32), int(t_now), float(dt_unit), n, out)
+    return out
+
+
+def correct(active, pos_pred, acc_new, t_now: int, dt_unit: float, pos_m, vel, acc_pot, t_last, level=None,
+            eps: float = 0.0, eta: float = 0.5, e_min: int = 0, max_levels: int = 8):
+    """O8, eq. 17 for the active i-particles, IN PLACE on pos_m, vel, acc_pot, t_last (and level: reading R15)."""
+    for a, dt in ((pos_m, np.float32), (vel, np.float32), (acc_pot, np.float32), (t_last, np.uint32)):
+        assert a.dtype == dt and a.flags.c_contiguous
+    active = np.ascontiguousarray(active, np.uint32)
+    lev_p = None
+    if level is not None:
+        assert level.dtype == np.uint8 and level.flags.c_contiguous
+        lev_p = level.ctypes.data_as(C.c_void_p)
+    lib().oracle_correct(active, active.shape[0], np.ascontiguousarray(pos_pred, np.float32), np.ascontiguousarray(acc_new, np.float32),
+                         int(t_now), float(dt_unit), pos_m, vel, acc_pot, t_last, lev_p,
+                         float(timestep_constant(eps, eta)) if level is not None else 0.0, int(e_min), int(max_levels))

@@ -498,4 +498,52 @@ void oracle_group_ball(const float *pos_sorted, const uint32_t *members, uint32_
     ball4[0] = rI[0]; ball4[1] = rI[1]; ball4[2] = rI[2]; ball4[3] = sqrtf(b2max);
 }
 
+/* O8 (NEXT row f1; section 2.7, eq. 15-17): second-order predictor-corrector under block time steps.
+ * Every particle j carries its state (r, v, a) at its own last corrected time t_last[j], counted in units of dt_unit
+ * (the finest step 2^e_min, so the float product below is exact).  Prediction of ALL j-particles to t_now:
+ *   dt = (t_now - t_last[j]) dt_unit;  v^{n+1/2} = v^n + (dt/2) a^n  (eq. 15);  r^{n+1} = r^n + dt v^{n+1/2}  (eq. 16).
+ * Single precision, one fused multiply-add per component, in this order (R15). */
+void oracle_predict(const float *pos_m, const float *vel, const float *acc_pot, const uint32_t *t_last, uint32_t t_now,
+                    float dt_unit, uint32_t n, float *pos_pred)
+{
+    for (uint32_t j = 0; j < n; j++) {
+        const float dt = (float)(t_now - t_last[j]) * dt_unit;
+        const float h = 0.5f * dt;
+        for (int k = 0; k < 3; k++) {
+            const float vh = fmaf(h, acc_pot[4 * (size_t)j + k], vel[4 * (size_t)j + k]);        /* eq. 15 */
+            pos_pred[4 * (size_t)j + k] = fmaf(dt, vh, pos_m[4 * (size_t)j + k]);                /* eq. 16 */
+        }
+        pos_pred[4 * (size_t)j + 3] = pos_m[4 * (size_t)j + 3];                                  /* mass */
+    }
+}
+
+/* Correction of the active i-particles (eq. 17): v^{n+1} = v^{n+1/2} + (dt/2) a^{n+1}, with v^{n+1/2} of eq. 15 over the
+ * particle's own full step; the predicted position becomes the particle's position, a^{n+1} its acceleration and t_now its
+ * time.  Level migration (the paper is silent; reading R15): the level wanted by the new acceleration is
+ * clamp(dt_exponent(a^{n+1}) - e_min, 0, max_levels - 1); a particle may move to any FINER level at once, and ONE level coarser
+ * only when t_now is a multiple of that coarser step (so that every particle stays aligned with its block).  level == NULL: none. */
+void oracle_correct(const uint32_t *active, uint32_t n_active, const float *pos_pred, const float *acc_new, uint32_t t_now,
+                    float dt_unit, float *pos_m, float *vel, float *acc_pot, uint32_t *t_last, uint8_t *level, float c,
+                    int e_min, int max_levels)
+{
+    for (uint32_t q = 0; q < n_active; q++) {
+        const size_t i = active[q];
+        const float dt = (float)(t_now - t_last[i]) * dt_unit;
+        const float h = 0.5f * dt;
+        for (int k = 0; k < 3; k++) {
+            const float vh = fmaf(h, acc_pot[4 * i + k], vel[4 * i + k]);                         /* eq. 15 */
+            vel[4 * i + k] = fmaf(h, acc_new[4 * i + k], vh);                                    /* eq. 17 */
+        }
+        for (int k = 0; k < 4; k++) { pos_m[4 * i + k] = pos_pred[4 * i + k]; acc_pot[4 * i + k] = acc_new[4 * i + k]; }
+        t_last[i] = t_now;
+        if (level) {
+            int want = dt_exponent(acc_new + 4 * i, c) - e_min;
+            want = std::max(0, std::min(want, max_levels - 1));
+            const int cur = level[i];
+            if (want < cur) level[i] = (uint8_t)want;
+            else if (want > cur && t_now % (1u << (cur + 1)) == 0) level[i] = (uint8_t)(cur + 1);
+        }
+    }
+}
+
 } /* extern "C" */
