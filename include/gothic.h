@@ -151,6 +151,31 @@ int gothic_block_cycle_host(gothic_ctx *ctx, const float *pos_m_host, const floa
                             int n_leaf, float eps, float eta, int max_levels, float delta_acc, float r_crit, float *acc_pot_host,
                             uint8_t *level_host, int32_t *info_host, unsigned long long *n_interactions_host, void *stream);
 
+/* Orbit integration under block time steps, section 2.7 (second-order predictor-corrector; NEXT row f1).
+ * Every particle carries (r, v, a) at its own last corrected time t_last, an integer count of dt_unit = 2^e_min (the finest
+ * step, {e_min, n_levels} from gothic_set_timesteps).  All arrays share ONE index space of the caller's choice (normally
+ * the sorted order of the last build).  Single precision, one fused multiply-add per component (R15).
+ *
+ * gothic_predict: eq. 15-16 for ALL n j-particles: dt = (t_now - t_last[j]) dt_unit, v' = v + (dt/2) a, r' = r + dt v'.
+ *   pos_m float4[n], vel float4[n] (vx,vy,vz,unused), acc_pot float4[n], t_last uint32[n]: in;  pos_pred float4[n]: out
+ *   (x,y,z predicted, mass copied).  t_now >= every t_last.  Asynchronous; 68 B per particle. */
+int gothic_predict(gothic_ctx *ctx, const float *pos_m, const float *vel, const float *acc_pot, const uint32_t *t_last,
+                   uint32_t t_now, float dt_unit, uint32_t n, float *pos_pred, void *stream);
+
+/* gothic_correct: eq. 17 for the ACTIVE i-particles (ascending indices as produced by gothic_set_timesteps):
+ * v <- (v + (dt/2) a_old) + (dt/2) a_new, r <- pos_pred, a <- acc_new, t_last <- t_now; other particles untouched.
+ *   active uint32[n_active] (NULL -> all n); n_active_dev optional device count overriding n_active.
+ *   pos_pred, acc_new float4[n]: in (acc_new = output of gothic_walk_tree for this substep; must not alias acc_pot).
+ *   pos_m, vel, acc_pot float4[n], t_last uint32[n]: in/out.
+ *   level uint8[n] in/out, or NULL for no level migration.  With level: the level the new acceleration asks for is
+ *   clamp(floor(log2(eta sqrt(eps/|a_new|))) - e_min, 0, max_levels-1) (same arithmetic as gothic_set_timesteps, R6);
+ *   a particle moves to any FINER level at once and ONE level coarser only when t_now is a multiple of that coarser
+ *   step (reading R15; the paper does not describe the migration).  Asynchronous. */
+int gothic_correct(gothic_ctx *ctx, const uint32_t *active, uint32_t n_active, const uint32_t *n_active_dev, uint32_t n,
+                   const float *pos_pred, const float *acc_new, uint32_t t_now, float dt_unit, float *pos_m, float *vel,
+                   float *acc_pot, uint32_t *t_last, uint8_t *level, float eps, float eta, int e_min, int max_levels,
+                   void *stream);
+
 /* Number of kernels this library has launched through this context (bench.py "gpu_launches"). */
 unsigned long long gothic_launch_count(gothic_ctx *ctx);
 

@@ -19,7 +19,7 @@ MAC_ACCELERATION, MAC_OPENING_ANGLE = 0, 1
 EXPORTS = [
     "gothic_create", "gothic_destroy", "gothic_strerror", "gothic_last_cuda_error", "gothic_build_tree",
     "gothic_update_moments", "gothic_walk_tree", "gothic_set_timesteps", "gothic_get_tree_view", "gothic_check",
-    "gothic_gravity_host", "gothic_block_cycle_host", "gothic_launch_count",
+    "gothic_gravity_host", "gothic_block_cycle_host", "gothic_launch_count", "gothic_predict", "gothic_correct",
 ]
 
 
@@ -72,6 +72,10 @@ def load_library():
     L.gothic_gravity_host.argtypes = [vp, vp, u32, i32, i32, f32, i32, f32, f32, vp, vp, vp, vp]
     L.gothic_block_cycle_host.restype = i32
     L.gothic_block_cycle_host.argtypes = [vp, vp, vp, u32, i32, i32, f32, f32, i32, f32, f32, vp, vp, vp, vp, vp]
+    L.gothic_predict.restype = i32
+    L.gothic_predict.argtypes = [vp, vp, vp, vp, vp, u32, f32, u32, vp, vp]
+    L.gothic_correct.restype = i32
+    L.gothic_correct.argtypes = [vp, vp, u32, vp, u32, vp, vp, u32, f32, vp, vp, vp, vp, vp, f32, f32, i32, i32, vp]
     L.gothic_launch_count.restype = C.c_ulonglong
     L.gothic_launch_count.argtypes = [vp]
     _lib = L
@@ -163,6 +167,23 @@ class Gothic:
         self._chk(self._L.gothic_set_timesteps(self._ctx, _ptr(acc_pot, torch.float32), level.shape[0], float(eps), float(eta),
                                                max_levels, substep, _ptr(level, torch.uint8), _ptr(active, torch.int32),
                                                _ptr(n_active_dev, torch.int32), _ptr(emin_nlev_dev, torch.int32), _stream()))
+
+    def predict(self, pos_m: torch.Tensor, vel: torch.Tensor, acc_pot: torch.Tensor, t_last: torch.Tensor, pos_pred: torch.Tensor, *,
+                t_now: int, dt_unit: float):
+        self._chk(self._L.gothic_predict(self._ctx, _ptr(pos_m, torch.float32), _ptr(vel, torch.float32), _ptr(acc_pot, torch.float32),
+                                         _ptr(t_last, torch.int32), int(t_now), float(dt_unit), pos_m.shape[0], _ptr(pos_pred, torch.float32), _stream()))
+
+    def correct(self, pos_pred: torch.Tensor, acc_new: torch.Tensor, pos_m: torch.Tensor, vel: torch.Tensor, acc_pot: torch.Tensor,
+                t_last: torch.Tensor, *, t_now: int, dt_unit: float, active: torch.Tensor | None = None, n_active: int | None = None,
+                n_active_dev: torch.Tensor | None = None, level: torch.Tensor | None = None, eps: float = 0.0, eta: float = 0.5,
+                e_min: int = 0, max_levels: int = 8):
+        na = 0
+        if active is not None:
+            na = int(active.shape[0] if n_active is None else n_active)
+        self._chk(self._L.gothic_correct(self._ctx, _ptr(active, torch.int32) if active is not None else None, na, _ptr(n_active_dev, torch.int32),
+                                         pos_m.shape[0], _ptr(pos_pred, torch.float32), _ptr(acc_new, torch.float32), int(t_now), float(dt_unit),
+                                         _ptr(pos_m, torch.float32), _ptr(vel, torch.float32), _ptr(acc_pot, torch.float32), _ptr(t_last, torch.int32),
+                                         _ptr(level, torch.uint8), float(eps), float(eta), int(e_min), int(max_levels), _stream()))
 
     def check(self):
         self._chk(self._L.gothic_check(self._ctx, _stream()))

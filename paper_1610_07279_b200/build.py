@@ -15,7 +15,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libgothic_b200.so")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
-SOURCES = ["gothic_api.cu", "build_keys.cu", "sort_pairs.cu", "build_nodes.cu", "moments.cu", "timesteps.cu", "walk.cu"]
+SOURCES = ["gothic_api.cu", "build_keys.cu", "sort_pairs.cu", "build_nodes.cu", "moments.cu", "timesteps.cu", "walk.cu", "integrate.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-I", INCLUDE]
 
