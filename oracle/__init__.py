@@ -52,7 +52,9 @@ def lib():
         L.oracle_direct.restype = None
         L.oracle_direct.argtypes = [_f32p, C.c_uint32, C.c_void_p, C.c_uint32, C.c_double, _f64p]
         L.oracle_walk.restype = None
-        L.oracle_walk.argtypes = [_f32p, C.c_uint32, _u32p, _u32p, _u32p, _u8p, _f32p, _f32p,
+        L.oracle_b2.restype = None
+        L.oracle_b2.argtypes = [_f32p, C.c_uint32, _u32p, _u32p, _f32p, _f32p]
+        L.oracle_walk.argtypes = [_f32p, C.c_uint32, _u32p, _u32p, _u32p, _u8p, _f32p, _f32p, C.c_void_p,
                                   C.c_void_p, C.c_uint32, C.c_int, C.c_float, C.c_int, C.c_float, C.c_void_p,
                                   C.c_uint32, C.c_uint32, C.c_float, _f64p, _u64p]
         L.oracle_predict.restype = None
@@ -216,8 +218,17 @@ def direct(pos_m, eps: float, targets=None) -> np.ndarray:
     return out
 
 
+def b2(pos_sorted, head, num, com) -> np.ndarray:
+    """O5b, eq. 4: B_2 about the given stored centres."""
+    m = head.shape[0]
+    out = np.zeros(m, np.float32)
+    lib().oracle_b2(_pos(pos_sorted), m, np.ascontiguousarray(head, np.uint32), np.ascontiguousarray(num, np.uint32),
+                    np.ascontiguousarray(com, np.float32), out)
+    return out
+
+
 def walk(pos_sorted, head, num, child, nchild, com, b, *, eps: float, mac_kind: int, mac_param: float,
-         aold=None, active=None, group_size: int = 32, group_range=None, r_crit: float = float("inf")):
+         aold=None, active=None, group_size: int = 32, group_range=None, r_crit: float = float("inf"), B2=None):
     """O7.  Returns (out float64 [n,4] (only active rows written), counts dict).
     r_crit: critical separation of P:122-126 (reading R13); inf = no group splitting."""
     pos_sorted = _pos(pos_sorted)
@@ -226,6 +237,12 @@ def walk(pos_sorted, head, num, child, nchild, com, b, *, eps: float, mac_kind: 
     counts = np.zeros(4, np.uint64)
     if mac_kind == 0 and aold is None:
         raise ValueError("acceleration MAC needs aold")
+    if mac_kind == 2 and B2 is None:
+        raise ValueError("multipole MAC needs B2")
+    b2_p = None
+    if B2 is not None:
+        B2 = np.ascontiguousarray(B2, np.float32)
+        b2_p = B2.ctypes.data_as(C.c_void_p)
     aold_p = None
     if aold is not None:
         aold = np.ascontiguousarray(aold, np.float32)
@@ -239,13 +256,15 @@ def walk(pos_sorted, head, num, child, nchild, com, b, *, eps: float, mac_kind: 
     lib().oracle_walk(pos_sorted, n,
                       np.ascontiguousarray(head, np.uint32), np.ascontiguousarray(num, np.uint32),
                       np.ascontiguousarray(child, np.uint32), np.ascontiguousarray(nchild, np.uint8),
-                      np.ascontiguousarray(com, np.float32), np.ascontiguousarray(b, np.float32),
+                      np.ascontiguousarray(com, np.float32), np.ascontiguousarray(b, np.float32), b2_p,
                       act_p, n_act, group_size, float(eps), mac_kind, float(mac_param), aold_p,
                       int(g_lo), int(g_hi), float(r_crit), out, counts)
     return out, dict(interactions=int(counts[0]), mac_tests=int(counts[1]), groups=int(counts[2]), list_entries=int(counts[3]))
 
 
 def walk_tree(t: Tree, **kw):
+    if kw.get("mac_kind") == 2 and "B2" not in kw:
+        kw["B2"] = b2(t.pos_sorted, t.head, t.num, t.com)
     return walk(t.pos_sorted, t.head, t.num, t.child, t.nchild, t.com, t.b, **kw)
 
 

@@ -261,6 +261,22 @@ void oracle_moments(const float *pos_sorted, uint32_t n_nodes, const uint32_t *h
     }
 }
 
+/* O5b (NEXT row f3; eq. 4): B_2 = sum_j m_j |r_j - r_J|^2 over the cell's particles about a GIVEN stored centre,
+ * accumulated in double, rounded once. */
+void oracle_b2(const float *pos_sorted, uint32_t n_nodes, const uint32_t *head, const uint32_t *num, const float *com4, float *B2)
+{
+#pragma omp parallel for schedule(dynamic, 256)
+    for (int64_t J = 0; J < (int64_t)n_nodes; J++) {
+        double acc = 0.0;
+        for (uint32_t j = head[J]; j < head[J] + num[J]; j++) {
+            const float *p = pos_sorted + 4 * (size_t)j;
+            const double dx = (double)p[0] - com4[4 * J], dy = (double)p[1] - com4[4 * J + 1], dz = (double)p[2] - com4[4 * J + 2];
+            acc += (double)p[3] * (dx * dx + dy * dy + dz * dz);
+        }
+        B2[J] = (float)acc;
+    }
+}
+
 /* O5, second half only: b_J = max |r_j - r_J| about a GIVEN stored centre com4 (stage-wise parity: the radius a
  * CUDA build reports is checked against the definition applied to the centre that same build stored). */
 void oracle_radius(const float *pos_sorted, uint32_t n_nodes, const uint32_t *head, const uint32_t *num,
@@ -360,7 +376,7 @@ void oracle_group_ball(const float *pos_sorted, const uint32_t *members, uint32_
  *           member is left; every piece then walks the tree on its own.  r_crit = INFINITY: no splitting (R3 as is). */
 void oracle_walk(const float *pos_sorted, uint32_t n,
                  const uint32_t *head, const uint32_t *num, const uint32_t *child, const uint8_t *nchild,
-                 const float *com4, const float *bJ,
+                 const float *com4, const float *bJ, const float *B2 /* eq. 4; needed iff mac_kind == 2 */,
                  const uint32_t *active, uint32_t n_active, int G,
                  float eps, int mac_kind, float mac_param, const float *aold,
                  uint32_t group_lo, uint32_t group_hi, float r_crit,
@@ -439,8 +455,14 @@ void oracle_walk(const float *pos_sorted, uint32_t n,
                 if (mac_kind == 0) {
                     const float mb2 = (com4[4 * (size_t)J + 3] * bJ[J]) * bJ[J];
                     accept = thr * ((d * d) * (d * d)) >= mb2; /* eq. 5, both sides to the 4th power */
-                } else {
+                } else if (mac_kind == 1) {
                     accept = bJ[J] <= thr * d;                 /* eq. 2 */
+                } else {
+                    /* eq. 3: d >= b/2 + sqrt(b^2/4 + sqrt(3 B_2 / Delta_mul)).  Since the right side is >= b, squaring
+                     * d - b/2 gives d (d - b) >= sqrt(3 B_2 / Delta), i.e. d >= b and Delta (d (d - b))^2 >= 3 B_2: the form
+                     * both sides evaluate in fp32 (R16; equivalence pinned in tests/test_oracle_multipole.py). */
+                    const float t = d * (d - bJ[J]);
+                    accept = d >= bJ[J] && thr * (t * t) >= 3.0f * B2[J];
                 }
             }
             if (accept) cells.push_back(J);
