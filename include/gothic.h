@@ -41,7 +41,7 @@ enum {
 };
 
 enum { GOTHIC_KEY_PEANO_HILBERT = 0, GOTHIC_KEY_MORTON = 1 };   /* PAPER.md:54 / PAPER.md:564 */
-enum { GOTHIC_MAC_ACCELERATION = 0, GOTHIC_MAC_OPENING_ANGLE = 1 }; /* eq. 5 PAPER.md:85-89 / eq. 2 */
+enum { GOTHIC_MAC_ACCELERATION = 0, GOTHIC_MAC_OPENING_ANGLE = 1, GOTHIC_MAC_MULTIPOLE = 2 }; /* eq. 5 PAPER.md:85-89 / eq. 2 PAPER.md:68-72 / eq. 3-4 */
 
 /* Allocates a context for up to n_max particles.
  *   node_max      node pool capacity; 0 -> 2*n_max (+64).  Must be < 2^28.
@@ -120,6 +120,7 @@ typedef struct {
     const uint32_t *level_ofs;    /* [23] device: id of the first node of each level */
     const float *node_com;        /* float4[n_nodes]: r_J, m_J */
     const float *node_b;          /* [n_nodes]: b_J */
+    const float *node_b2;         /* [n_nodes]: B_2 = sum_j m_j |r_j - r_J|^2 (eq. 4) */
 } gothic_tree_view;
 int gothic_get_tree_view(gothic_ctx *ctx, gothic_tree_view *out, void *stream);
 

@@ -14,7 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libgothic_b200.so")
 
 KEY_PEANO_HILBERT, KEY_MORTON = 0, 1
-MAC_ACCELERATION, MAC_OPENING_ANGLE = 0, 1
+MAC_ACCELERATION, MAC_OPENING_ANGLE, MAC_MULTIPOLE = 0, 1, 2
 
 EXPORTS = [
     "gothic_create", "gothic_destroy", "gothic_strerror", "gothic_last_cuda_error", "gothic_build_tree",
@@ -33,7 +33,7 @@ class TreeViewStruct(C.Structure):
                 ("key", C.c_void_p), ("perm", C.c_void_p), ("pos_m_sorted", C.c_void_p),
                 ("node_head", C.c_void_p), ("node_num", C.c_void_p), ("node_child", C.c_void_p),
                 ("node_level", C.c_void_p), ("node_nchild", C.c_void_p), ("level_ofs", C.c_void_p),
-                ("node_com", C.c_void_p), ("node_b", C.c_void_p)]
+                ("node_com", C.c_void_p), ("node_b", C.c_void_p), ("node_b2", C.c_void_p)]
 
 
 _lib = None
@@ -204,7 +204,7 @@ class Gothic:
             node_head=_from_ptr(v.node_head, m, torch.int32, d), node_num=_from_ptr(v.node_num, m, torch.int32, d),
             node_child=_from_ptr(v.node_child, m, torch.int32, d), node_level=_from_ptr(v.node_level, m, torch.uint8, d),
             node_nchild=_from_ptr(v.node_nchild, m, torch.uint8, d), level_ofs=_from_ptr(v.level_ofs, 23, torch.int32, d),
-            node_com=_from_ptr(v.node_com, 4 * m, torch.float32, d).view(m, 4), node_b=_from_ptr(v.node_b, m, torch.float32, d),
+            node_com=_from_ptr(v.node_com, 4 * m, torch.float32, d).view(m, 4), node_b=_from_ptr(v.node_b, m, torch.float32, d), node_b2=_from_ptr(v.node_b2, m, torch.float32, d),
         )
 
     def gravity_host(self, pos_m_host: torch.Tensor, acc_pot_host: torch.Tensor, *, eps: float, mac_kind: int, mac_param: float,

@@ -15,7 +15,7 @@
 // FAMILY the walk pushes when it opens the node: first item, count | particles << 31.
 struct __align__(16) NodeRec {
     float x, y, z, m;   // r_J, m_J
-    float mb2;          // (m_J * b_J) * b_J   (eq. 5 right-hand side numerator, G = 1)
+    float mb2;          // (m_J * b_J) * b_J (eq. 5 right-hand side, G = 1); 3 B_2 while the multipole MAC is in use (eq. 3)
     float b;            // b_J
     uint32_t w0;        // internal: item of the first child's record (n_max + 2 * child) | leaf: head (sorted index of first particle)
     uint32_t w1;        // internal: number of children                                    | leaf: 0x80000000 | num
@@ -50,6 +50,9 @@ struct gothic_ctx {
     float4 *node_up;       // (r_J, parent id as bits): one 16-byte load per level of the radius climb
     uint32_t *leaf_of;     // [n_max] leaf node of every sorted particle
     float *node_b;
+    float *node_B2;        // eq. 4: sum_j m_j |r_j - r_J|^2 (multipole MAC)
+    bool b2_enabled;       // the moments passes of this context also compute B_2
+    int rec_slot4;         // what NodeRec::mb2 holds now: GOTHIC_MAC_ACCELERATION -> m b^2, GOTHIC_MAC_MULTIPOLE -> 3 B_2
     uint32_t *node_b2bits;
     NodeRec *node_rec;     // = items + n_max
     uint32_t *level_ofs;   // [23]
@@ -96,6 +99,8 @@ size_t gothic_sort_scratch_bytes(uint32_t n_max);
 int gothic_stage_gather(gothic_ctx *c, const float4 *pos_m, uint32_t n, cudaStream_t s);
 int gothic_stage_nodes(gothic_ctx *c, uint32_t n, int n_leaf, cudaStream_t s);
 int gothic_stage_moments(gothic_ctx *c, cudaStream_t s);
+int gothic_stage_need_b2(gothic_ctx *c, cudaStream_t s);   // computes B_2 now if this context has not been asked for it before
+int gothic_stage_rec_slot4(gothic_ctx *c, int mac_kind, cudaStream_t s);   // switches NodeRec::mb2 between m b^2 and 3 B_2
 int gothic_stage_walk(gothic_ctx *c, const uint32_t *active, uint32_t n_active, const uint32_t *n_active_dev,
                       float eps, int mac_kind, float mac_param, float r_crit, const float *aold, float4 *acc_pot,
                       float *amag_out, unsigned long long *n_inter, cudaStream_t s);

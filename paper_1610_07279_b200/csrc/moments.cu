@@ -32,7 +32,7 @@ __device__ __forceinline__ float4 com_of(float4 ms)
 __global__ void __launch_bounds__(TPB) k_leaf_moments(uint32_t n_nodes, const float4 *__restrict__ pos, const uint32_t *__restrict__ node_head,
                                                        const uint32_t *__restrict__ node_num, const uint32_t *__restrict__ node_child,
                                                        float4 *__restrict__ node_msum, float4 *__restrict__ node_com, uint32_t *__restrict__ node_b2bits,
-                                                       const uint32_t *__restrict__ node_parent, float4 *__restrict__ node_up)
+                                                       const uint32_t *__restrict__ node_parent, float4 *__restrict__ node_up, float *__restrict__ node_B2)
 {
     const uint32_t J = blockIdx.x * TPB + threadIdx.x;
     if (J >= n_nodes || node_child[J] != GOTHIC_LEAF) return;
@@ -40,6 +40,7 @@ __global__ void __launch_bounds__(TPB) k_leaf_moments(uint32_t n_nodes, const fl
     if (c == 1) {   // a single-particle node IS the particle (bitwise), b_J = 0
         const float4 p = __ldg(pos + h);
         store_com(J, make_float4(p.w * p.x, p.w * p.y, p.w * p.z, p.w), p, node_msum, node_com, node_b2bits, node_parent, node_up);
+        if (node_B2) node_B2[J] = 0.0f;
         return;
     }
     float4 ms = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -47,13 +48,22 @@ __global__ void __launch_bounds__(TPB) k_leaf_moments(uint32_t n_nodes, const fl
         const float4 p = __ldg(pos + j);
         ms.x = fmaf(p.w, p.x, ms.x); ms.y = fmaf(p.w, p.y, ms.y); ms.z = fmaf(p.w, p.z, ms.z); ms.w += p.w;
     }
-    store_com(J, ms, com_of(ms), node_msum, node_com, node_b2bits, node_parent, node_up);
+    const float4 cm = com_of(ms);
+    store_com(J, ms, cm, node_msum, node_com, node_b2bits, node_parent, node_up);
+    if (!node_B2) return;
+    float B2 = 0.0f;                                     // eq. 4 about the stored centre
+    for (uint32_t j = h; j < h + c; j++) {
+        const float4 p = __ldg(pos + j);
+        const float dx = p.x - cm.x, dy = p.y - cm.y, dz = p.z - cm.z;
+        B2 = fmaf(p.w, fmaf(dz, dz, fmaf(dy, dy, dx * dx)), B2);
+    }
+    node_B2[J] = B2;
 }
 
 __global__ void __launch_bounds__(TPB) k_internal_moments(uint32_t first, uint32_t count, const uint32_t *__restrict__ node_child,
                                                            const uint8_t *__restrict__ node_nchild, float4 *__restrict__ node_msum,
                                                            float4 *__restrict__ node_com, uint32_t *__restrict__ node_b2bits,
-                                                           const uint32_t *__restrict__ node_parent, float4 *__restrict__ node_up)
+                                                           const uint32_t *__restrict__ node_parent, float4 *__restrict__ node_up, float *__restrict__ node_B2)
 {
     const uint32_t t = blockIdx.x * TPB + threadIdx.x;
     if (t >= count) return;
@@ -65,7 +75,16 @@ __global__ void __launch_bounds__(TPB) k_internal_moments(uint32_t first, uint32
         const float4 q = node_msum[c + k];
         ms.x += q.x; ms.y += q.y; ms.z += q.z; ms.w += q.w;
     }
-    store_com(J, ms, com_of(ms), node_msum, node_com, node_b2bits, node_parent, node_up);
+    const float4 cm = com_of(ms);
+    store_com(J, ms, cm, node_msum, node_com, node_b2bits, node_parent, node_up);
+    if (!node_B2) return;
+    float B2 = 0.0f;                                     // parallel-axis theorem over the children: B2_c + m_c |r_c - r_J|^2
+    for (uint32_t k = 0; k < nc; k++) {
+        const float4 q = node_com[c + k];
+        const float dx = q.x - cm.x, dy = q.y - cm.y, dz = q.z - cm.z;
+        B2 += fmaf(q.w, fmaf(dz, dz, fmaf(dy, dy, dx * dx)), node_B2[c + k]);
+    }
+    node_B2[J] = B2;
 }
 
 // Persistent warps, each sweeping a contiguous range of sorted particles 32 at a time.  Lane L of a warp remembers the
@@ -176,18 +195,51 @@ __global__ void __launch_bounds__(TPB) k_pack_nodes(uint32_t n_nodes, const uint
     rec[J] = r;
 }
 
+// NodeRec::mb2 <- m b^2 (acceleration MAC, eq. 5) or 3 B_2 (multipole MAC, eq. 3): one 4-byte store per node
+__global__ void __launch_bounds__(TPB) k_rec_slot4(uint32_t n_nodes, int multipole, const float4 *__restrict__ node_com, const float *__restrict__ node_b,
+                                                    const float *__restrict__ node_B2, NodeRec *__restrict__ rec)
+{
+    const uint32_t J = blockIdx.x * TPB + threadIdx.x;
+    if (J >= n_nodes) return;
+    if (multipole) rec[J].mb2 = __fmul_rn(3.0f, node_B2[J]);
+    else { const float b = node_b[J]; rec[J].mb2 = __fmul_rn(__fmul_rn(node_com[J].w, b), b); }
+}
+
 } // namespace
+
+// B_2 (eq. 4) is only computed once somebody has asked for it (multipole MAC or tree view); from then on every moments pass of
+// this context carries it along.
+int gothic_stage_need_b2(gothic_ctx *c, cudaStream_t s)
+{
+    if (c->b2_enabled) return GOTHIC_OK;
+    c->b2_enabled = true;
+    return gothic_stage_moments(c, s);
+}
+
+int gothic_stage_rec_slot4(gothic_ctx *c, int mac_kind, cudaStream_t s)
+{
+    const int want = mac_kind == GOTHIC_MAC_MULTIPOLE ? GOTHIC_MAC_MULTIPOLE : GOTHIC_MAC_ACCELERATION;
+    if (mac_kind == GOTHIC_MAC_OPENING_ANGLE || c->rec_slot4 == want) return GOTHIC_OK;     // eq. 2 reads b_J only
+    if (want == GOTHIC_MAC_MULTIPOLE) {
+        const int rc = gothic_stage_need_b2(c, s);
+        if (rc != GOTHIC_OK) return rc;
+    }
+    k_rec_slot4<<<(c->n_nodes + TPB - 1) / TPB, TPB, 0, s>>>(c->n_nodes, want == GOTHIC_MAC_MULTIPOLE, c->node_com, c->node_b, c->node_B2, c->node_rec);
+    GOTHIC_LAUNCH_OK(c);
+    c->rec_slot4 = want;
+    return GOTHIC_OK;
+}
 
 int gothic_stage_moments(gothic_ctx *c, cudaStream_t s)
 {
     const uint32_t m = c->n_nodes;
     const uint32_t grid = (m + TPB - 1) / TPB;
-    k_leaf_moments<<<grid, TPB, 0, s>>>(m, c->pos_sorted, c->node_head, c->node_num, c->node_child, c->node_msum, c->node_com, c->node_b2bits, c->node_parent, c->node_up);
+    k_leaf_moments<<<grid, TPB, 0, s>>>(m, c->pos_sorted, c->node_head, c->node_num, c->node_child, c->node_msum, c->node_com, c->node_b2bits, c->node_parent, c->node_up, c->b2_enabled ? c->node_B2 : nullptr);
     GOTHIC_LAUNCH_OK(c);
     for (int L = (int)c->n_levels_tree - 2; L >= 0; L--) {
         const uint32_t first = c->h_level_ofs[L], count = c->h_level_ofs[L + 1] - first;
         if (!count) continue;
-        k_internal_moments<<<(count + TPB - 1) / TPB, TPB, 0, s>>>(first, count, c->node_child, c->node_nchild, c->node_msum, c->node_com, c->node_b2bits, c->node_parent, c->node_up);
+        k_internal_moments<<<(count + TPB - 1) / TPB, TPB, 0, s>>>(first, count, c->node_child, c->node_nchild, c->node_msum, c->node_com, c->node_b2bits, c->node_parent, c->node_up, c->b2_enabled ? c->node_B2 : nullptr);
         GOTHIC_LAUNCH_OK(c);
     }
     {
@@ -201,5 +253,6 @@ int gothic_stage_moments(gothic_ctx *c, cudaStream_t s)
     GOTHIC_LAUNCH_OK(c);
     k_pack_nodes<<<grid, TPB, 0, s>>>(m, c->node_head, c->node_num, c->node_child, c->node_nchild, c->node_com, c->node_b2bits, c->node_b, c->node_rec, c->n_max);
     GOTHIC_LAUNCH_OK(c);
+    c->rec_slot4 = GOTHIC_MAC_ACCELERATION;
     return GOTHIC_OK;
 }

@@ -194,3 +194,43 @@ def test_walk_full_size_hernquist_sampled(oracle):
     assert mom < 2e-3 and np.all(out[:, 3] < 0)
     assert 1000 < cnt / n < 2500
     g.close()
+
+
+@pytest.mark.parametrize("model,n,G,frac,r_crit", [("plummer", 1 << 13, 32, 1.0, float("inf")), ("nfw", 30000, 16, 0.3, 0.2),
+                                                     ("m31_like", 40001, 32, 1.0, 0.5), ("hernquist", 20000, 8, 0.05, float("inf"))])
+def test_walk_multipole_mac_matches_oracle(oracle, model, n, G, frac, r_crit):
+    """NEXT row f3: the multipole MAC of eq. 3-4.  B_2 from the CUDA moments pass is held against the definition,
+    then the oracle walks with the SAME B_2, so decisions and interaction counts must be equal."""
+    from gpu_util import gpu_build, gpu_walk
+    pos = getattr(W, model)(n, seed=8)
+    eps = 2.0 ** -7
+    g, v = gpu_build(pos, group_size=G)
+    B2_def = oracle.b2(v["pos_m_sorted"], v["node_head"], v["node_num"], v["node_com"])
+    assert np.all(np.abs(v["node_b2"] - B2_def) <= 1e-3 * B2_def + 1e-12)
+    assert np.all(v["node_b2"][v["node_num"] == 1] == 0)
+    active = None if frac == 1.0 else W.random_active_subset(n, frac, seed=3)
+    rows = np.arange(n) if active is None else active
+    aold = np.ones(n, np.float32)
+    for dmul in (2.0 ** -2, 2.0 ** -8, 2.0 ** -14):
+        out, cnt, _ = gpu_walk(g, n, eps=eps, mac_kind=2, mac_param=dmul, active=active, r_crit=r_crit)
+        ref, c = _oracle_on_gpu_tree(oracle, v, eps=eps, mac_kind=2, mac_param=dmul, active=active, group_size=G, r_crit=r_crit, B2=v["node_b2"])
+        assert cnt == c["interactions"]
+        _assert_parity(out, ref, rows)
+        # switching MACs back and forth re-packs the record slot: the acceleration MAC must be unaffected
+        out0, cnt0, _ = gpu_walk(g, n, eps=eps, mac_kind=0, mac_param=2.0 ** -7, aold=aold, active=active, r_crit=r_crit)
+        ref0, c0 = _oracle_on_gpu_tree(oracle, v, eps=eps, mac_kind=0, mac_param=2.0 ** -7, aold=aold, active=active, group_size=G, r_crit=r_crit)
+        assert cnt0 == c0["interactions"]
+        _assert_parity(out0, ref0, rows)
+    g.close()
+
+
+def test_multipole_mac_error_vs_direct_sum(oracle):
+    """Error against eq. 1 in double falls as Delta_mul tightens (Fig. 3 blue squares)."""
+    from gpu_util import gpu_build, gpu_walk, acc_rel_err
+    n = 20000
+    pos = W.plummer(n, seed=5)
+    g, v = gpu_build(pos)
+    direct = oracle.direct(v["pos_m_sorted"], 1.0 / 64)
+    med = [float(np.median(acc_rel_err(gpu_walk(g, n, eps=1.0 / 64, mac_kind=2, mac_param=2.0 ** -e)[0], direct))) for e in (-2, 3, 8, 13)]
+    assert all(b < a for a, b in zip(med, med[1:])) and med[0] > 1e-3 and med[-1] < 3e-4, med
+    g.close()
