@@ -56,14 +56,14 @@ def lib():
         L.oracle_b2.argtypes = [_f32p, C.c_uint32, _u32p, _u32p, _f32p, _f32p]
         L.oracle_walk.argtypes = [_f32p, C.c_uint32, _u32p, _u32p, _u32p, _u8p, _f32p, _f32p, C.c_void_p,
                                   C.c_void_p, C.c_uint32, C.c_int, C.c_float, C.c_int, C.c_float, C.c_void_p,
-                                  C.c_uint32, C.c_uint32, C.c_float, _f64p, _u64p]
+                                  C.c_uint32, C.c_uint32, C.c_float, C.c_int, _f64p, _u64p]
         L.oracle_predict.restype = None
         L.oracle_predict.argtypes = [_f32p, _f32p, _f32p, _u32p, C.c_uint32, C.c_float, C.c_uint32, _f32p]
         L.oracle_correct.restype = None
         L.oracle_correct.argtypes = [_u32p, C.c_uint32, _f32p, _f32p, C.c_uint32, C.c_float, _f32p, _f32p, _f32p, _u32p,
                                      C.c_void_p, C.c_float, C.c_int, C.c_int]
         L.oracle_group_ball.restype = None
-        L.oracle_group_ball.argtypes = [_f32p, _u32p, C.c_uint32, _f32p]
+        L.oracle_group_ball.argtypes = [_f32p, _u32p, C.c_uint32, C.c_int, _f32p]
         _lib = L
     return _lib
 
@@ -228,7 +228,7 @@ def b2(pos_sorted, head, num, com) -> np.ndarray:
 
 
 def walk(pos_sorted, head, num, child, nchild, com, b, *, eps: float, mac_kind: int, mac_param: float,
-         aold=None, active=None, group_size: int = 32, group_range=None, r_crit: float = float("inf"), B2=None):
+         aold=None, active=None, group_size: int = 32, group_range=None, r_crit: float = float("inf"), B2=None, ball_kind: int = 0):
     """O7.  Returns (out float64 [n,4] (only active rows written), counts dict).
     r_crit: critical separation of P:122-126 (reading R13); inf = no group splitting."""
     pos_sorted = _pos(pos_sorted)
@@ -258,7 +258,7 @@ def walk(pos_sorted, head, num, child, nchild, com, b, *, eps: float, mac_kind: 
                       np.ascontiguousarray(child, np.uint32), np.ascontiguousarray(nchild, np.uint8),
                       np.ascontiguousarray(com, np.float32), np.ascontiguousarray(b, np.float32), b2_p,
                       act_p, n_act, group_size, float(eps), mac_kind, float(mac_param), aold_p,
-                      int(g_lo), int(g_hi), float(r_crit), out, counts)
+                      int(g_lo), int(g_hi), float(r_crit), int(ball_kind), out, counts)
     return out, dict(interactions=int(counts[0]), mac_tests=int(counts[1]), groups=int(counts[2]), list_entries=int(counts[3]))
 
 
@@ -268,10 +268,11 @@ def walk_tree(t: Tree, **kw):
     return walk(t.pos_sorted, t.head, t.num, t.child, t.nchild, t.com, t.b, **kw)
 
 
-def group_ball(pos_sorted, members) -> np.ndarray:
+def group_ball(pos_sorted, members, ball_kind: int = 0) -> np.ndarray:
+    """(r_I, b_I) as the walk forms it: ball_kind 0 = GEO, 1 = EBS (Ritter), App. B P:568."""
     out = np.zeros(4, np.float32)
     members = np.ascontiguousarray(members, np.uint32)
-    lib().oracle_group_ball(_pos(pos_sorted), members, members.shape[0], out)
+    lib().oracle_group_ball(_pos(pos_sorted), members, members.shape[0], int(ball_kind), out)
     return out
 
 

@@ -359,7 +359,61 @@ void oracle_direct(const float *pos_m, uint32_t n, const uint32_t *targets, uint
     }
 }
 
-void oracle_group_ball(const float *pos_sorted, const uint32_t *members, uint32_t k, float *ball4);
+void oracle_group_ball(const float *pos_sorted, const uint32_t *members, uint32_t k, int ball_kind, float *ball4);
+
+static inline float dist2f(const float *a, const float *b)
+{
+    const float dx = a[0] - b[0], dy = a[1] - b[1], dz = a[2] - b[2];
+    return fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+}
+
+/* Centre of the pseudo i-particle's enclosing ball (App. B).  The radius is then always the exact maximum distance
+ * of the members from that centre.
+ *   ball_kind 0, GEO (item 3): centre of the bounding rectangular cuboid.
+ *   ball_kind 1, EBS (item 2): Ritter's efficient bounding sphere (1990).  Pass 1: the first members (ascending order) that
+ *     attain the minimum and the maximum of each coordinate; of the three pairs the one farthest apart (x before y before z on
+ *     ties) spans the first sphere: centre = midpoint, radius = distance from the centre to the pair's maximum point.  Pass 2,
+ *     members in ascending order: a point at distance dist > r grows the sphere just enough to contain it and the old sphere:
+ *     r' = (r + dist)/2, centre moves by (dist - r')/dist of the way to the point.  fp32, operations as written (R17). */
+static void ball_centre(const float *pos_sorted, const uint32_t *members, uint32_t k, int ball_kind, float rI[3])
+{
+    if (ball_kind == 0) {
+        float lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+        for (uint32_t q = 0; q < k; q++)
+            for (int d = 0; d < 3; d++) {
+                lo[d] = std::min(lo[d], pos_sorted[4 * (size_t)members[q] + d]);
+                hi[d] = std::max(hi[d], pos_sorted[4 * (size_t)members[q] + d]);
+            }
+        for (int d = 0; d < 3; d++) rI[d] = 0.5f * (lo[d] + hi[d]);
+        return;
+    }
+    uint32_t imin[3] = {0, 0, 0}, imax[3] = {0, 0, 0};
+    for (uint32_t q = 1; q < k; q++)
+        for (int d = 0; d < 3; d++) {
+            const float v = pos_sorted[4 * (size_t)members[q] + d];
+            if (v < pos_sorted[4 * (size_t)members[imin[d]] + d]) imin[d] = q;
+            if (v > pos_sorted[4 * (size_t)members[imax[d]] + d]) imax[d] = q;
+        }
+    int a = 0;
+    float best = -1.0f;
+    for (int d = 0; d < 3; d++) {
+        const float s2 = dist2f(pos_sorted + 4 * (size_t)members[imax[d]], pos_sorted + 4 * (size_t)members[imin[d]]);
+        if (s2 > best) { best = s2; a = d; }
+    }
+    const float *pa = pos_sorted + 4 * (size_t)members[imin[a]], *pb = pos_sorted + 4 * (size_t)members[imax[a]];
+    for (int d = 0; d < 3; d++) rI[d] = 0.5f * (pa[d] + pb[d]);
+    float r2 = dist2f(pb, rI), r = sqrtf(r2);
+    for (uint32_t q = 0; q < k; q++) {
+        const float *p = pos_sorted + 4 * (size_t)members[q];
+        const float dx = p[0] - rI[0], dy = p[1] - rI[1], dz = p[2] - rI[2];
+        const float d2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+        if (d2 > r2) {
+            const float dist = sqrtf(d2), rn = 0.5f * (r + dist), f = (dist - rn) / dist;
+            rI[0] = fmaf(f, dx, rI[0]); rI[1] = fmaf(f, dy, rI[1]); rI[2] = fmaf(f, dz, rI[2]);
+            r = rn; r2 = rn * rn;
+        }
+    }
+}
 
 /* O7 (P:105-118 traversal with a pseudo i-particle; eq. 5; eq. 2; P:62 monopole).
  * One group = aligned chunk of G consecutive sorted indices (reading R3); members = its active particles;
@@ -379,7 +433,7 @@ void oracle_walk(const float *pos_sorted, uint32_t n,
                  const float *com4, const float *bJ, const float *B2 /* eq. 4; needed iff mac_kind == 2 */,
                  const uint32_t *active, uint32_t n_active, int G,
                  float eps, int mac_kind, float mac_param, const float *aold,
-                 uint32_t group_lo, uint32_t group_hi, float r_crit,
+                 uint32_t group_lo, uint32_t group_hi, float r_crit, int ball_kind /* 0 GEO, 1 EBS (App. B) */,
                  double *out4, uint64_t *counts)
 {
     const uint32_t n_groups = (n + (uint32_t)G - 1) / (uint32_t)G;
@@ -409,7 +463,7 @@ void oracle_walk(const float *pos_sorted, uint32_t n,
             todo.pop_back();
             const uint32_t cnt = pr.second - pr.first;
             float ball[4];
-            oracle_group_ball(pos_sorted, K.data() + pr.first, cnt, ball);
+            oracle_group_ball(pos_sorted, K.data() + pr.first, cnt, ball_kind, ball);
             if (cnt > 1 && ball[3] > r_crit) {
                 const uint32_t mid = pr.first + (cnt + 1) / 2;
                 todo.push_back(std::make_pair(mid, pr.second));
@@ -419,18 +473,11 @@ void oracle_walk(const float *pos_sorted, uint32_t n,
         const std::vector<uint32_t> Kall = K;
         for (const std::pair<uint32_t, uint32_t> &pc : pieces) {
         K.assign(Kall.begin() + pc.first, Kall.begin() + pc.second);
-        /* pseudo i-particle: GEO ball (App. B P:568 item 3) */
-        float lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+        /* pseudo i-particle: enclosing ball (App. B; GEO item 3 or EBS item 2) and a_min over the members */
         float amin = INFINITY;
-        for (uint32_t k : K) {
-            for (int d = 0; d < 3; d++) {
-                lo[d] = std::min(lo[d], pos_sorted[4 * (size_t)k + d]);
-                hi[d] = std::max(hi[d], pos_sorted[4 * (size_t)k + d]);
-            }
-            if (aold) amin = std::min(amin, aold[k]);
-        }
+        if (aold) for (uint32_t k : K) amin = std::min(amin, aold[k]);
         float rI[3];
-        for (int d = 0; d < 3; d++) rI[d] = 0.5f * (lo[d] + hi[d]);
+        ball_centre(pos_sorted, K.data(), (uint32_t)K.size(), ball_kind, rI);
         float b2max = 0.0f;
         for (uint32_t k : K) {
             const float dx = pos_sorted[4 * (size_t)k] - rI[0], dy = pos_sorted[4 * (size_t)k + 1] - rI[1],
@@ -501,16 +548,10 @@ void oracle_walk(const float *pos_sorted, uint32_t n,
 }
 
 /* P:118 pin helper: for one group, the ball (r_I, b_I) exactly as oracle_walk forms it. */
-void oracle_group_ball(const float *pos_sorted, const uint32_t *members, uint32_t k, float *ball4)
+void oracle_group_ball(const float *pos_sorted, const uint32_t *members, uint32_t k, int ball_kind, float *ball4)
 {
-    float lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
-    for (uint32_t q = 0; q < k; q++)
-        for (int d = 0; d < 3; d++) {
-            lo[d] = std::min(lo[d], pos_sorted[4 * (size_t)members[q] + d]);
-            hi[d] = std::max(hi[d], pos_sorted[4 * (size_t)members[q] + d]);
-        }
     float rI[3];
-    for (int d = 0; d < 3; d++) rI[d] = 0.5f * (lo[d] + hi[d]);
+    ball_centre(pos_sorted, members, k, ball_kind, rI);
     float b2max = 0.0f;
     for (uint32_t q = 0; q < k; q++) {
         const float dx = pos_sorted[4 * (size_t)members[q]] - rI[0], dy = pos_sorted[4 * (size_t)members[q] + 1] - rI[1],

@@ -1,0 +1,69 @@
+"""Pins for the enclosing balls of the pseudo i-particle (App. B): GEO and Ritter's EBS.  Independent facts:
+every member is inside; special cases with known answers; the smallest enclosing ball (found here by an independent
+iteration in double) bounds both from below, and EBS stays within the ~10 % Ritter claims and the paper repeats."""
+import numpy as np
+
+import oracle
+
+
+def _pts(k, rng, scale=1.0):
+    p = np.zeros((k, 4), np.float32)
+    p[:, :3] = rng.normal(size=(k, 3)) * scale + rng.normal(size=3)
+    p[:, 3] = 1.0
+    return p
+
+
+def _seb_radius(x, iters=4000):
+    """Badoiu-Clarkson: move the centre 1/(i+1) of the way to the farthest point; converges to the smallest enclosing ball."""
+    c = x[0].copy()
+    for i in range(1, iters):
+        far = x[np.argmax(((x - c) ** 2).sum(1))]
+        c += (far - c) / (i + 1)
+    return np.sqrt(((x - c) ** 2).sum(1).max())
+
+
+def test_members_are_enclosed_and_radius_is_the_exact_maximum():
+    rng = np.random.default_rng(1)
+    for k in (1, 2, 3, 5, 17, 32):
+        for kind in (0, 1):
+            p = _pts(k, rng, scale=10.0 ** rng.uniform(-3, 1))
+            ball = oracle.group_ball(p, np.arange(k), kind)
+            d = np.sqrt(((p[:, :3].astype(np.float64) - ball[:3].astype(np.float64)) ** 2).sum(1))
+            assert np.all(d <= ball[3] * (1 + 2e-7) + 1e-30)
+            assert np.isclose(d.max(), ball[3], rtol=3e-7, atol=1e-30)
+
+
+def test_special_cases():
+    one = np.array([[1.5, -2.0, 3.0, 1.0]], np.float32)
+    two = np.array([[0, 0, 0, 1], [2, 4, 4, 1]], np.float32)                       # distance 6
+    line = np.zeros((9, 4), np.float32)
+    line[:, 0] = np.arange(9)                                                      # collinear: diameter 8
+    for kind in (0, 1):
+        b = oracle.group_ball(one, [0], kind)
+        assert np.array_equal(b[:3], one[0, :3]) and b[3] == 0
+        b = oracle.group_ball(two, [0, 1], kind)
+        assert np.allclose(b, [1, 2, 2, 3], atol=1e-6)
+        b = oracle.group_ball(line, np.arange(9), kind)
+        assert np.allclose(b, [4, 0, 0, 4], atol=1e-6)
+    # members are a SUBSET of the array: only they count
+    rng = np.random.default_rng(2)
+    p = _pts(40, rng)
+    mem = np.array([3, 7, 8, 20, 31], np.uint32)
+    for kind in (0, 1):
+        assert np.array_equal(oracle.group_ball(p, mem, kind), oracle.group_ball(p[mem], np.arange(5), kind))
+
+
+def test_radii_against_the_smallest_enclosing_ball():
+    """EBS "overestimation is 5% in most cases and ~10% in the worst case"; GEO "smaller than 1.15 r_SEB in most cases"."""
+    rng = np.random.default_rng(3)
+    ratios = {0: [], 1: []}
+    for _ in range(300):
+        k = int(rng.integers(4, 33))
+        p = _pts(k, rng)
+        seb = _seb_radius(p[:, :3].astype(np.float64))
+        for kind in (0, 1):
+            ratios[kind].append(oracle.group_ball(p, np.arange(k), kind)[3] / seb)
+    geo, ebs = np.array(ratios[0]), np.array(ratios[1])
+    assert geo.min() > 1 - 2e-3 and ebs.min() > 1 - 2e-3               # nothing beats the smallest ball (iteration tolerance)
+    assert np.median(ebs) < 1.08 and ebs.max() < 1.25
+    assert np.median(geo) < 1.15 and np.median(ebs) < np.median(geo)   # EBS is the tighter of the two (Fig. B.10)
