@@ -15,11 +15,12 @@ LIB_PATH = os.path.join(_HERE, "libgothic_b200.so")
 
 KEY_PEANO_HILBERT, KEY_MORTON = 0, 1
 MAC_ACCELERATION, MAC_OPENING_ANGLE, MAC_MULTIPOLE = 0, 1, 2
+BALL_GEO, BALL_EBS = 0, 1
 
 EXPORTS = [
     "gothic_create", "gothic_destroy", "gothic_strerror", "gothic_last_cuda_error", "gothic_build_tree",
     "gothic_update_moments", "gothic_walk_tree", "gothic_set_timesteps", "gothic_get_tree_view", "gothic_check",
-    "gothic_gravity_host", "gothic_block_cycle_host", "gothic_launch_count", "gothic_predict", "gothic_correct",
+    "gothic_gravity_host", "gothic_block_cycle_host", "gothic_launch_count", "gothic_predict", "gothic_correct", "gothic_set_ball",
 ]
 
 
@@ -72,6 +73,8 @@ def load_library():
     L.gothic_gravity_host.argtypes = [vp, vp, u32, i32, i32, f32, i32, f32, f32, vp, vp, vp, vp]
     L.gothic_block_cycle_host.restype = i32
     L.gothic_block_cycle_host.argtypes = [vp, vp, vp, u32, i32, i32, f32, f32, i32, f32, f32, vp, vp, vp, vp, vp]
+    L.gothic_set_ball.restype = i32
+    L.gothic_set_ball.argtypes = [vp, i32]
     L.gothic_predict.restype = i32
     L.gothic_predict.argtypes = [vp, vp, vp, vp, vp, u32, f32, u32, vp, vp]
     L.gothic_correct.restype = i32
@@ -184,6 +187,9 @@ class Gothic:
                                          pos_m.shape[0], _ptr(pos_pred, torch.float32), _ptr(acc_new, torch.float32), int(t_now), float(dt_unit),
                                          _ptr(pos_m, torch.float32), _ptr(vel, torch.float32), _ptr(acc_pot, torch.float32), _ptr(t_last, torch.int32),
                                          _ptr(level, torch.uint8), float(eps), float(eta), int(e_min), int(max_levels), _stream()))
+
+    def set_ball(self, ball_kind: int):
+        self._chk(self._L.gothic_set_ball(self._ctx, int(ball_kind)))
 
     def check(self):
         self._chk(self._L.gothic_check(self._ctx, _stream()))

@@ -146,6 +146,13 @@ void gothic_destroy(gothic_ctx *ctx)
     delete ctx;
 }
 
+int gothic_set_ball(gothic_ctx *ctx, int ball_kind)
+{
+    if (!ctx || (ball_kind != GOTHIC_BALL_GEO && ball_kind != GOTHIC_BALL_EBS)) return GOTHIC_ERR_ARG;
+    ctx->ball_kind = ball_kind;
+    return GOTHIC_OK;
+}
+
 unsigned long long gothic_launch_count(gothic_ctx *ctx) { return ctx ? ctx->launches : 0ull; }
 
 int gothic_build_tree(gothic_ctx *c, const float *pos_m, uint32_t n, int key_kind, int n_leaf, void *stream)

@@ -24,6 +24,7 @@ struct __align__(16) NodeRec {
 struct gothic_ctx {
     uint32_t n_max, node_max;
     int group_size;
+    int ball_kind;         // enclosing ball of the pseudo i-particle: GOTHIC_BALL_GEO (default) or GOTHIC_BALL_EBS
     int n_leaf;
     int device;
     int num_sms;

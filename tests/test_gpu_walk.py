@@ -234,3 +234,31 @@ def test_multipole_mac_error_vs_direct_sum(oracle):
     med = [float(np.median(acc_rel_err(gpu_walk(g, n, eps=1.0 / 64, mac_kind=2, mac_param=2.0 ** -e)[0], direct))) for e in (-2, 3, 8, 13)]
     assert all(b < a for a, b in zip(med, med[1:])) and med[0] > 1e-3 and med[-1] < 3e-4, med
     g.close()
+
+
+@pytest.mark.parametrize("model,n,G,frac,r_crit", [("plummer", 1 << 13, 32, 1.0, float("inf")), ("nfw", 30011, 32, 0.3, 0.3),
+                                                     ("m31_like", 20000, 16, 1.0, 0.5), ("hernquist", 20000, 8, 0.04, float("inf"))])
+def test_walk_ebs_ball_matches_oracle(oracle, model, n, G, frac, r_crit):
+    """NEXT row f3: Ritter's efficient bounding sphere as the pseudo i-particle (App. B item 2).  The ball decides every MAC and
+    the r_crit splitting, so centre arithmetic is bit-for-bit the oracle's: interaction counts must be equal."""
+    from gpu_util import gpu_build, gpu_walk
+    from paper_1610_07279_b200.binding import BALL_EBS, BALL_GEO
+    pos = getattr(W, model)(n, seed=9)
+    eps = 2.0 ** -7
+    g, v = gpu_build(pos, group_size=G)
+    aold = _bootstrap_aold(g, n, eps)
+    active = None if frac == 1.0 else W.random_active_subset(n, frac, seed=2)
+    rows = np.arange(n) if active is None else active
+    g.set_ball(BALL_EBS)
+    counts = {}
+    for kind, param in ((0, 2.0 ** -8), (1, 0.6), (2, 2.0 ** -6)):
+        out, cnt, _ = gpu_walk(g, n, eps=eps, mac_kind=kind, mac_param=param, aold=aold, active=active, r_crit=r_crit)
+        ref, c = _oracle_on_gpu_tree(oracle, v, eps=eps, mac_kind=kind, mac_param=param, aold=aold, active=active, group_size=G,
+                                     r_crit=r_crit, ball_kind=1, B2=v["node_b2"])
+        assert cnt == c["interactions"]
+        _assert_parity(out, ref, rows)
+        counts[kind] = cnt
+    g.set_ball(BALL_GEO)
+    _, cnt_geo, _ = gpu_walk(g, n, eps=eps, mac_kind=0, mac_param=2.0 ** -8, aold=aold, active=active, r_crit=r_crit)
+    assert counts[0] != cnt_geo and abs(counts[0] - cnt_geo) < 0.1 * cnt_geo       # a different, slightly tighter ball
+    g.close()
