@@ -22,6 +22,8 @@ void free_all(gothic_ctx *c)
                     c->h2d_acc, c->d_level, c->d_active, c->d_cycle_info, c->d_count};
     for (void *p : ptrs)
         if (p) cudaFree(p);
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+    if (c->copy_done) cudaEventDestroy(c->copy_done);
 }
 
 __global__ void k_gather_f32(const float *__restrict__ src, const uint32_t *__restrict__ perm, uint32_t n, float *__restrict__ dst)
@@ -315,10 +317,19 @@ int gothic_block_cycle_host(gothic_ctx *c, const float *pos_m_host, const float 
         if (e != cudaSuccess) { c->last_err = e; return GOTHIC_ERR_CUDA; }
     }
     const size_t b4 = (size_t)n * sizeof(float4);
+    if (!c->copy_stream) {
+        GOTHIC_CUDA_OK(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+        GOTHIC_CUDA_OK(c, cudaEventCreateWithFlags(&c->copy_done, cudaEventDisableTiming));
+    }
+    // the build needs only the positions: the previous accelerations travel on a second queue while the tree is built
     GOTHIC_CUDA_OK(c, cudaMemcpyAsync(c->h2d_pos, pos_m_host, b4, cudaMemcpyHostToDevice, s));
-    GOTHIC_CUDA_OK(c, cudaMemcpyAsync(c->h2d_acc, acc_prev_host, b4, cudaMemcpyHostToDevice, s));
+    GOTHIC_CUDA_OK(c, cudaEventRecord(c->copy_done, s));
+    GOTHIC_CUDA_OK(c, cudaStreamWaitEvent(c->copy_stream, c->copy_done, 0));     // after the positions (one H2D engine) and after earlier work on s
+    GOTHIC_CUDA_OK(c, cudaMemcpyAsync(c->h2d_acc, acc_prev_host, b4, cudaMemcpyHostToDevice, c->copy_stream));
+    GOTHIC_CUDA_OK(c, cudaEventRecord(c->copy_done, c->copy_stream));
     int rc = gothic_build_tree(c, reinterpret_cast<const float *>(c->h2d_pos), n, key_kind, n_leaf, stream);
     if (rc != GOTHIC_OK) return rc;
+    GOTHIC_CUDA_OK(c, cudaStreamWaitEvent(s, c->copy_done, 0));
     const uint32_t grid = (n + 255u) / 256u;
     float *amag = c->d_aold_sorted;
     uint8_t *level = c->d_level, *level_orig = c->d_level + c->n_max;

@@ -76,6 +76,7 @@ struct gothic_ctx {
     uint32_t *scan_tmp;    // block counts for ordered compaction
     // host staging for gothic_gravity_host
     float4 *h2d_pos; float *h2d_aold; float *d_aold_sorted; float4 *d_acc;
+    cudaStream_t copy_stream; cudaEvent_t copy_done;   // second copy queue of gothic_block_cycle_host (overlaps H2D with the build)
     // extra staging for gothic_block_cycle_host
     float4 *h2d_acc; uint8_t *d_level; uint32_t *d_active; int32_t *d_cycle_info; unsigned long long *d_count;
 };
