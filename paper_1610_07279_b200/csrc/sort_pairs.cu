@@ -79,7 +79,7 @@ struct SortSmem {
     uint32_t tile;
 };
 
-__global__ void __launch_bounds__(SORT_TPB) k_sort_onesweep(const uint64_t *__restrict__ kin, const uint32_t *__restrict__ vin,
+__global__ void __launch_bounds__(SORT_TPB, 3) k_sort_onesweep(const uint64_t *__restrict__ kin, const uint32_t *__restrict__ vin,
                                                             uint64_t *__restrict__ kout, uint32_t *__restrict__ vout, uint32_t n, int shift,
                                                             const uint32_t *__restrict__ gstart, uint32_t *__restrict__ ticket,
                                                             volatile uint32_t *status)
@@ -114,11 +114,12 @@ __global__ void __launch_bounds__(SORT_TPB) k_sort_onesweep(const uint64_t *__re
         const uint32_t d = (uint32_t)(k[i] >> shift) & 255u;
         const uint32_t peers = __match_any_sync(FULL, valid ? d : 256u);
         const int leader = __ffs(peers) - 1;
+        // one returning shared-memory atomic per distinct digit of the row: atomics of one warp on one address complete in
+        // program order, so the rows need no barrier between them and their latencies overlap
         uint32_t old = 0;
-        if ((int)lane == leader && valid) { old = S.hist[warp][d]; S.hist[warp][d] = old + __popc(peers); }
+        if ((int)lane == leader && valid) old = atomicAdd(&S.hist[warp][d], (uint32_t)__popc(peers));
         old = __shfl_sync(FULL, old, leader);
         pos[i] = old + __popc(peers & lt);
-        __syncwarp();
     }
     __syncthreads();
 
@@ -147,6 +148,8 @@ __global__ void __launch_bounds__(SORT_TPB) k_sort_onesweep(const uint64_t *__re
         for (uint32_t w = 0; w < warp; w++) wbase += S.wsum[w];
         const uint32_t excl = wbase + incl - count;
         S.dstart[tid] = excl;
+#pragma unroll
+        for (int w = 0; w < SORT_WARPS; w++) S.hist[w][tid] += excl;       // slot of (warp, digit, rank) = hist[warp][digit] + rank
         // decoupled look-back: sum of this digit's counts over tiles tile-1, tile-2, ... until an inclusive one
         uint32_t prefix = 0;
         if (tile > 0) {
@@ -169,7 +172,7 @@ __global__ void __launch_bounds__(SORT_TPB) k_sort_onesweep(const uint64_t *__re
         const uint32_t j = warp * (32u * IPT) + (uint32_t)i * 32u + lane;
         if (j < n_valid) {
             const uint32_t d = (uint32_t)(k[i] >> shift) & 255u;
-            const uint32_t p = S.dstart[d] + S.hist[warp][d] + pos[i];
+            const uint32_t p = S.hist[warp][d] + pos[i];
             S.keys[p] = k[i];
             S.vals[p] = v[i];
         }
@@ -201,6 +204,7 @@ int gothic_stage_sort(gothic_ctx *c, uint32_t n, cudaStream_t s)
     static bool configured = false;
     if (!configured) {
         cudaFuncSetAttribute(k_sort_onesweep, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem));
+        cudaFuncSetAttribute(k_sort_onesweep, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
         configured = true;
     }
     const uint32_t ntiles = (n + TILE - 1) / TILE;
