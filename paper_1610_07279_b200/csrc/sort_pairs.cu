@@ -199,14 +199,14 @@ size_t gothic_sort_scratch_bytes(uint32_t n_max)
     return (sort_words_head() + (size_t)NPASS * ntiles * RADIX) * sizeof(uint32_t);
 }
 
+void gothic_sort_config()
+{
+    cudaFuncSetAttribute(k_sort_onesweep, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem));
+    cudaFuncSetAttribute(k_sort_onesweep, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+}
+
 int gothic_stage_sort(gothic_ctx *c, uint32_t n, cudaStream_t s)
 {
-    static bool configured = false;
-    if (!configured) {
-        cudaFuncSetAttribute(k_sort_onesweep, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem));
-        cudaFuncSetAttribute(k_sort_onesweep, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-        configured = true;
-    }
     const uint32_t ntiles = (n + TILE - 1) / TILE;
     uint32_t *words = static_cast<uint32_t *>(c->sort_tmp);
     uint32_t *ghist = words, *ticket = words + NPASS * RADIX, *status = words + sort_words_head();
