@@ -99,6 +99,7 @@ int gothic_create(gothic_ctx **out, uint32_t n_max, uint32_t node_max, int group
     if (e != cudaSuccess) { c->last_err = e; delete c; *out = nullptr; return GOTHIC_ERR_CUDA; }
     gothic_walk_config(c);
     gothic_sort_config();
+    if (gothic_keys_config(c) != GOTHIC_OK) { delete c; *out = nullptr; return GOTHIC_ERR_CUDA; }
     c->stack_cap = 8192;   // u32 words of global spill area per resident warp (4096 families)
     if (scratch_bytes) {
         const size_t per = scratch_bytes / ((size_t)c->walk_warps * sizeof(uint32_t));

@@ -98,6 +98,7 @@ struct gothic_ctx {
 int gothic_stage_keys(gothic_ctx *c, const float4 *pos_m, uint32_t n, int key_kind, cudaStream_t s);
 int gothic_stage_sort(gothic_ctx *c, uint32_t n, cudaStream_t s);
 size_t gothic_sort_scratch_bytes(uint32_t n_max);
+int gothic_keys_config(gothic_ctx *c);     // uploads the Peano-Hilbert state table (called by gothic_create)
 void gothic_sort_config();                // per-device function attributes of the sort kernels (called by gothic_create)
 int gothic_stage_gather(gothic_ctx *c, const float4 *pos_m, uint32_t n, cudaStream_t s);
 int gothic_stage_nodes(gothic_ctx *c, uint32_t n, int n_leaf, cudaStream_t s);
