@@ -221,7 +221,8 @@ __global__ void __launch_bounds__(TPB) k_emit_nodes(const uint64_t *__restrict__
 __global__ void __launch_bounds__(TPB) k_finish_nodes(uint32_t n_nodes, const uint32_t *__restrict__ node_head,
                                                        const uint32_t *__restrict__ node_end, const uint32_t *__restrict__ node_child,
                                                        const uint32_t *__restrict__ node_last, uint32_t *__restrict__ node_num,
-                                                       uint8_t *__restrict__ node_nchild, uint32_t *__restrict__ node_parent, uint32_t *__restrict__ leaf_of)
+                                                       uint8_t *__restrict__ node_nchild, uint32_t *__restrict__ node_parent, uint32_t *__restrict__ leaf_of,
+                                                       const uint8_t *__restrict__ node_level, uint8_t *__restrict__ leaf_level)
 {
     const uint32_t J = blockIdx.x * TPB + threadIdx.x;
     if (J >= n_nodes) return;
@@ -229,7 +230,10 @@ __global__ void __launch_bounds__(TPB) k_finish_nodes(uint32_t n_nodes, const ui
     node_num[J] = num;
     const uint32_t c = node_child[J];
     if (c == GOTHIC_LEAF)
-        for (uint32_t i = 0; i < num; i++) leaf_of[h + i] = J;
+    {
+        const uint8_t lv = node_level[J];
+        for (uint32_t i = 0; i < num; i++) { leaf_of[h + i] = J; leaf_level[h + i] = lv; }
+    }
     uint32_t nc = 0;
     if (c != GOTHIC_LEAF) {
         nc = node_last[J] - c + 1u;
@@ -266,7 +270,7 @@ int gothic_stage_nodes(gothic_ctx *c, uint32_t n, int n_leaf, cudaStream_t s)
     for (int L = 0; L < GOTHIC_NLEVP1; L++)
         if (c->h_level_ofs[L + 1] > c->h_level_ofs[L]) c->n_levels_tree = L + 1;
     k_finish_nodes<<<(c->n_nodes + TPB - 1) / TPB, TPB, 0, s>>>(c->n_nodes, c->node_head, c->node_end, c->node_child, c->node_last,
-                                                                c->node_num, c->node_nchild, c->node_parent, c->leaf_of);
+                                                                c->node_num, c->node_nchild, c->node_parent, c->leaf_of, c->node_level, c->leaf_level);
     GOTHIC_LAUNCH_OK(c);
     return GOTHIC_OK;
 }

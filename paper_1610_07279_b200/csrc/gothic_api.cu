@@ -16,7 +16,7 @@ void free_all(gothic_ctx *c)
 {
     void *ptrs[] = {c->key[0], c->key[1], c->idx[0], c->idx[1], c->items, c->box, c->bbox_bits,
                     c->node_head, c->node_num, c->node_child, c->node_parent, c->node_end, c->node_last,
-                    c->node_level, c->node_nchild, c->node_com, c->node_msum, c->node_b, c->node_B2, c->node_b2bits, c->node_up, c->leaf_of,
+                    c->node_level, c->node_nchild, c->node_com, c->node_msum, c->node_b, c->node_B2, c->node_b2bits, c->node_up, c->leaf_of, c->leaf_level,
                     c->level_ofs, c->level_cnt, c->blk_cnt, c->flags, c->sort_tmp, c->grp_mask, c->grp_list, c->grp_cnt,
                     c->stack, c->ts_tmp, c->scan_tmp, c->h2d_pos, c->h2d_aold, c->d_aold_sorted, c->d_acc,
                     c->h2d_acc, c->d_level, c->d_active, c->d_cycle_info, c->d_count};
@@ -119,7 +119,7 @@ int gothic_create(gothic_ctx **out, uint32_t n_max, uint32_t node_max, int group
     A(dev_alloc(&c->node_parent, m)); A(dev_alloc(&c->node_end, m)); A(dev_alloc(&c->node_last, m));
     A(dev_alloc(&c->node_level, m)); A(dev_alloc(&c->node_nchild, m));
     A(dev_alloc(&c->node_com, m)); A(dev_alloc(&c->node_msum, m)); A(dev_alloc(&c->node_b, m));
-    A(dev_alloc(&c->node_b2bits, m)); A(dev_alloc(&c->node_B2, m)); A(dev_alloc(&c->node_up, m)); A(dev_alloc(&c->leaf_of, n));
+    A(dev_alloc(&c->node_b2bits, m)); A(dev_alloc(&c->node_B2, m)); A(dev_alloc(&c->node_up, m)); A(dev_alloc(&c->leaf_of, n)); A(dev_alloc(&c->leaf_level, n));
     A(dev_alloc(&c->level_ofs, GOTHIC_NLEVP1 + 2)); A(dev_alloc(&c->level_cnt, GOTHIC_NLEVP1 + 2));
     A(dev_alloc(&c->blk_cnt, (size_t)2 * GOTHIC_NLEVP1 * c->nblk_max));
     A(dev_alloc(&c->flags, 4));

@@ -50,6 +50,7 @@ struct gothic_ctx {
     float4 *node_com, *node_msum;
     float4 *node_up;       // (r_J, parent id as bits): one 16-byte load per level of the radius climb
     uint32_t *leaf_of;     // [n_max] leaf node of every sorted particle
+    uint8_t *leaf_level;   // [n_max] and its level
     float *node_b;
     float *node_B2;        // eq. 4: sum_j m_j |r_j - r_J|^2 (multipole MAC)
     bool b2_enabled;       // the moments passes of this context also compute B_2

@@ -94,7 +94,7 @@ __global__ void __launch_bounds__(TPB) k_internal_moments(uint32_t first, uint32
 // maximum is written out (guarded atomicMax) when the warp moves on to another node of that level or finishes, so the
 // upper levels, which every particle contributes to, cost a few thousand atomics in total.
 __global__ void __launch_bounds__(TPB) k_node_radius(uint32_t n, uint32_t per_warp, const float4 *__restrict__ pos,
-                                                      const uint32_t *__restrict__ leaf_of, const uint8_t *__restrict__ node_level,
+                                                      const uint32_t *__restrict__ leaf_of, const uint8_t *__restrict__ leaf_level,
                                                       const uint32_t *__restrict__ node_head, const uint32_t *__restrict__ node_num,
                                                       const float4 *__restrict__ node_up, uint32_t *__restrict__ node_b2bits)
 {
@@ -106,19 +106,23 @@ __global__ void __launch_bounds__(TPB) k_node_radius(uint32_t n, uint32_t per_wa
     // lane L: level L
     uint32_t m_node = GOTHIC_LEAF, m_head = 0u, m_end = 0u, m_max = 0u;
     float m_x = 0.f, m_y = 0.f, m_z = 0.f;
-    // the next chunk's particle, leaf and leaf level are requested one chunk ahead
-    float4 p_nx = make_float4(0.f, 0.f, 0.f, 0.f);
+    // the next chunk's particle, leaf, leaf level (its own array: no dependent load) are requested one chunk ahead, and the
+    // leaf's own record as soon as its id is there
+    float4 p_nx = make_float4(0.f, 0.f, 0.f, 0.f), u_nx = make_float4(0.f, 0.f, 0.f, 0.f);
     uint32_t A_nx = GOTHIC_LEAF;
     int lev_nx = -1;
-    if ((uint32_t)r0 + lane < r1) { p_nx = __ldg(pos + (uint32_t)r0 + lane); A_nx = __ldg(leaf_of + (uint32_t)r0 + lane); lev_nx = node_level[A_nx]; }
+    if ((uint32_t)r0 + lane < r1) {
+        p_nx = __ldg(pos + (uint32_t)r0 + lane); A_nx = __ldg(leaf_of + (uint32_t)r0 + lane); lev_nx = __ldg(leaf_level + (uint32_t)r0 + lane);
+        u_nx = node_up[A_nx];
+    }
     for (uint32_t s0 = (uint32_t)r0; s0 < r1; s0 += 32u) {
         const uint32_t s = s0 + lane;
         const bool act = s < r1;
-        const float4 p = p_nx;
+        const float4 p = p_nx, u_leaf = u_nx;
         uint32_t A = A_nx;
         int lev = lev_nx;
         p_nx = make_float4(0.f, 0.f, 0.f, 0.f); A_nx = GOTHIC_LEAF; lev_nx = -1;
-        if (s + 32u < r1) { p_nx = __ldg(pos + s + 32u); A_nx = __ldg(leaf_of + s + 32u); lev_nx = node_level[A_nx]; }
+        if (s + 32u < r1) { p_nx = __ldg(pos + s + 32u); A_nx = __ldg(leaf_of + s + 32u); lev_nx = __ldg(leaf_level + s + 32u); }
         // ---- top-down over the levels whose remembered node contains the whole chunk (nested, so levels 0 .. Lf-1) ----
         const uint32_t in_mask = __ballot_sync(0xffffffffu, m_node != GOTHIC_LEAF && s0 >= m_head && min(s0 + 32u, r1) <= m_end);
         const int Lf = __ffs(~in_mask) - 1;
@@ -133,8 +137,8 @@ __global__ void __launch_bounds__(TPB) k_node_radius(uint32_t n, uint32_t per_wa
         //      level, so that the lanes that sit in the same node are neighbours; the record of the next level is
         //      requested before the reduction of this one ----
         int L = __reduce_max_sync(0xffffffffu, lev);
-        float4 u = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (lev == L && L >= Lf) u = node_up[A];
+        if (A_nx != GOTHIC_LEAF) u_nx = node_up[A_nx];          // the next chunk's leaf records, used one iteration from now
+        float4 u = u_leaf;                                      // a lane's first record is its leaf's, already here
         for (; L >= Lf; L--) {
             const bool on = lev == L;
             const uint32_t node = on ? A : GOTHIC_LEAF;
@@ -146,7 +150,7 @@ __global__ void __launch_bounds__(TPB) k_node_radius(uint32_t n, uint32_t per_wa
                 A = __float_as_uint(u.w);
                 lev = L - 1;
             }
-            if (lev == L - 1 && L > Lf) u = node_up[A];
+            if (on && L > Lf) u = node_up[A];                    // the parent's record; lanes that join later still hold their leaf's
             int all_same = 0;
             __match_all_sync(0xffffffffu, node, &all_same);
             if (all_same) {                                                  // whole chunk in one node: remember it
@@ -248,7 +252,7 @@ int gothic_stage_moments(gothic_ctx *c, cudaStream_t s)
         if (per_sm < 1) per_sm = 1;
         const uint32_t blocks = (uint32_t)(c->num_sms * per_sm), warps = blocks * (TPB / 32);     // one resident wave
         const uint32_t per_warp = (((c->n + warps - 1) / warps + 31u) / 32u) * 32u;
-        k_node_radius<<<blocks, TPB, 0, s>>>(c->n, per_warp, c->pos_sorted, c->leaf_of, c->node_level, c->node_head, c->node_num, c->node_up, c->node_b2bits);
+        k_node_radius<<<blocks, TPB, 0, s>>>(c->n, per_warp, c->pos_sorted, c->leaf_of, c->leaf_level, c->node_head, c->node_num, c->node_up, c->node_b2bits);
     }
     GOTHIC_LAUNCH_OK(c);
     k_pack_nodes<<<grid, TPB, 0, s>>>(m, c->node_head, c->node_num, c->node_child, c->node_nchild, c->node_com, c->node_b2bits, c->node_b, c->node_rec, c->n_max);
