@@ -416,7 +416,7 @@ static void ball_centre(const float *pos_sorted, const uint32_t *members, uint32
 }
 
 /* O7 (P:105-118 traversal with a pseudo i-particle; eq. 5; eq. 2; P:62 monopole).
- * One group = G consecutive entries of the ascending list of active particles (reading R3);
+ * One group = aligned chunk of G consecutive sorted indices (reading R3); members = its active particles;
  * GEO enclosing ball and a_min = min |a_old| over members (R4).  All MAC-deciding arithmetic in fp32 with
  * the operation order written here; the sums over the interaction list are in double.
  *   active == NULL  -> all n particles active.
@@ -436,18 +436,25 @@ void oracle_walk(const float *pos_sorted, uint32_t n,
                  uint32_t group_lo, uint32_t group_hi, float r_crit, int ball_kind /* 0 GEO, 1 EBS (App. B) */,
                  double *out4, uint64_t *counts)
 {
-    /* i-groups (reading R3, "whether to unify i-particles into a group or not"): the ascending list of ACTIVE particles
-     * (all n when active == NULL) is cut into consecutive chunks of G; chunk g = entries [G g, G g + G). */
-    const uint32_t n_list = active ? n_active : n;
-    const uint32_t n_groups = (n_list + (uint32_t)G - 1) / (uint32_t)G;
+    const uint32_t n_groups = (n + (uint32_t)G - 1) / (uint32_t)G;
     group_hi = std::min(group_hi, n_groups);
+    /* members per group from the ascending active list */
+    std::vector<uint32_t> first(n_groups + 1, 0);
+    if (active) {
+        for (uint32_t k = 0; k < n_active; k++) first[active[k] / G + 1]++;
+        for (uint32_t g = 0; g < n_groups; g++) first[g + 1] += first[g];
+    }
     const double eps2 = (double)eps * (double)eps;
     uint64_t c_int = 0, c_mac = 0, c_grp = 0, c_list = 0;
 
 #pragma omp parallel for schedule(dynamic, 16) reduction(+ : c_int, c_mac, c_grp, c_list)
     for (int64_t g = group_lo; g < (int64_t)group_hi; g++) {
         std::vector<uint32_t> K;
-        for (uint32_t q = (uint32_t)g * G; q < std::min(n_list, (uint32_t)(g + 1) * G); q++) K.push_back(active ? active[q] : q);
+        if (active) {
+            for (uint32_t k = first[g]; k < first[g + 1]; k++) K.push_back(active[k]);
+        } else {
+            for (uint32_t s = (uint32_t)g * G; s < std::min(n, (uint32_t)(g + 1) * G); s++) K.push_back(s);
+        }
         if (K.empty()) continue;
         /* §2.4 / R13: pieces of the member list, produced depth-first (first half before second half) */
         std::vector<std::pair<uint32_t, uint32_t>> todo(1, std::make_pair(0u, (uint32_t)K.size())), pieces;
