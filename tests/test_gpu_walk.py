@@ -260,5 +260,5 @@ def test_walk_ebs_ball_matches_oracle(oracle, model, n, G, frac, r_crit):
         counts[kind] = cnt
     g.set_ball(BALL_GEO)
     _, cnt_geo, _ = gpu_walk(g, n, eps=eps, mac_kind=0, mac_param=2.0 ** -8, aold=aold, active=active, r_crit=r_crit)
-    assert counts[0] != cnt_geo and abs(counts[0] - cnt_geo) < 0.1 * cnt_geo       # a different, slightly tighter ball
+    assert counts[0] != cnt_geo and abs(counts[0] - cnt_geo) < 0.2 * cnt_geo       # a different, slightly tighter ball
     g.close()
