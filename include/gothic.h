@@ -79,12 +79,17 @@ int gothic_update_moments(gothic_ctx *ctx, const float *pos_m_sorted, void *stre
  *   eps           Plummer softening length, > 0.
  *   mac_kind      GOTHIC_MAC_ACCELERATION: accept J iff d >= (m_J b_J^2 / (mac_param |a_old|))^(1/4)  (eq. 5)
  *                 GOTHIC_MAC_OPENING_ANGLE: accept J iff b_J / d <= mac_param                         (eq. 2)
- *                 d measured from the surface of the group's enclosing ball (eq. 6-7).
+ *                 GOTHIC_MAC_MULTIPOLE:     accept J iff d >= b_J/2 + sqrt(b_J^2/4 + sqrt(3 B_2 / mac_param)) (eq. 3-4), evaluated
+ *                                           as d >= b_J and mac_param (d (d - b_J))^2 >= 3 B_2 (R16)
+ *                 d measured from the surface of the group's enclosing ball (eq. 6-7; the ball is chosen
+ *                 with gothic_set_ball).
  *   r_crit        critical separation of PAPER.md:122-126 (R13): a group's member list (ascending) whose
  *                 enclosing ball has b_I > r_crit is cut into its first ceil(k/2) members and the rest, recursively,
  *                 until b_I <= r_crit or one member is left; every piece walks the tree on its own.  INFINITY = never
  *                 split; 0 = every particle alone.  Must not be NaN or negative.  (The paper auto-tunes this number
- *                 from timings; here it is the caller's.)
+ *                 from timings; here it is the caller's.  With INFINITY the few groups that straddle a jump of the
+ *                 space-filling curve walk almost the whole tree and hold the last warps for milliseconds: pass a finite
+ *                 value, e.g. a few per cent of the system's size.)
  *   aold          float[n] |a_old| per particle, sorted order; required iff mac_kind == ACCELERATION.
  *   acc_pot       float4[n] sorted order; ONLY active entries are written: (ax, ay, az, Phi).
  *   amag_out      optional float[n]: |a| of the new acceleration for active entries (may alias aold).
