@@ -21,8 +21,14 @@ constexpr int RADIX = 256;
 constexpr int NPASS = 8;                    // 8 x 8 bits >= 63
 constexpr int SORT_TPB = 256;
 constexpr int SORT_WARPS = SORT_TPB / 32;
-constexpr int IPT = 16;                     // items per thread
-constexpr int TILE = SORT_TPB * IPT;        // 4096 pairs per CTA
+#ifndef GOTHIC_SORT_IPT
+#define GOTHIC_SORT_IPT 16
+#endif
+#ifndef GOTHIC_SORT_CTAS
+#define GOTHIC_SORT_CTAS 3
+#endif
+constexpr int IPT = GOTHIC_SORT_IPT;        // items per thread
+constexpr int TILE = SORT_TPB * IPT;        // pairs per CTA (4096)
 constexpr uint32_t ST_AGG = 1u << 30;       // status word: this tile's own count is in the low 30 bits
 constexpr uint32_t ST_INC = 1u << 31;       //              the count of this and ALL earlier tiles is
 constexpr uint32_t ST_VAL = ST_AGG - 1u;
@@ -79,7 +85,7 @@ struct SortSmem {
     uint32_t tile;
 };
 
-__global__ void __launch_bounds__(SORT_TPB, 3) k_sort_onesweep(const uint64_t *__restrict__ kin, const uint32_t *__restrict__ vin,
+__global__ void __launch_bounds__(SORT_TPB, GOTHIC_SORT_CTAS) k_sort_onesweep(const uint64_t *__restrict__ kin, const uint32_t *__restrict__ vin,
                                                             uint64_t *__restrict__ kout, uint32_t *__restrict__ vout, uint32_t n, int shift,
                                                             const uint32_t *__restrict__ gstart, uint32_t *__restrict__ ticket,
                                                             volatile uint32_t *status)
