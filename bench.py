@@ -412,6 +412,11 @@ def run_ours(args, rank: int, world: int, local_rank: int):
                          "avg_launch_ms": stage_ms["walk"] / max(walk_launches, 1),
                          "peak_source": f"derived: {props.multi_processor_count} SM x 128 FP32 lanes x 2 flop x {peaks['sm_max_mhz']:.0f} MHz "
                                         f"(clock from MEASURED_PEAKS.json, {peaks['source']})"},
+            # the HBM-bound part: algorithmic bytes of one build (bbox 16, keys 16 + 8, histogram 8, 8 sort passes x 2 x 12,
+            # gather 4 + 16 + 16, node events 2 x 8 B per particle; moments 16 + 16 + 4 + 1 B per particle and ~150 B per node)
+            "build_roofline": {"bound": "hbm", "achieved": (n * 309 + 0.24 * n * 150) / (stage_ms["build"] / K * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
+                               "unit": "GB/s", "frac": (n * 309 + 0.24 * n * 150) / (stage_ms["build"] / K * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                               "ms": stage_ms["build"] / K, "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peaks['source']})"},
             "clocks": clk.summary(),
             "gpu_launches": int(launches),
             "e2e": None,
