@@ -262,3 +262,37 @@ def test_walk_ebs_ball_matches_oracle(oracle, model, n, G, frac, r_crit):
     _, cnt_geo, _ = gpu_walk(g, n, eps=eps, mac_kind=0, mac_param=2.0 ** -8, aold=aold, active=active, r_crit=r_crit)
     assert counts[0] != cnt_geo and abs(counts[0] - cnt_geo) < 0.2 * cnt_geo       # a different, slightly tighter ball
     g.close()
+
+
+def test_walk_edge_cases(oracle):
+    """Empty active set through the device count, all particles in one point, a massless particle, a far-offset system."""
+    from gpu_util import gpu_build, gpu_walk, dev
+    # device count = 0: nothing is written, nothing hangs
+    pos = W.plummer(1000, seed=2)
+    g, v = gpu_build(pos)
+    acc = torch.full((1000, 4), 7.0, device="cuda")
+    zero = torch.zeros(1, dtype=torch.int32, device="cuda")
+    g.walk_tree(acc, eps=0.05, mac_kind=1, mac_param=0.5, active=torch.zeros(10, dtype=torch.int32, device="cuda"), n_active_dev=zero)
+    g.check()
+    assert torch.all(acc == 7.0)
+    g.close()
+    # every particle at the same point: one level-21 leaf; a = 0, Phi = -(n-1) m / eps
+    n = 200
+    same = np.tile(np.array([[0.25, -1.5, 3.0, 0.5]], np.float32), (n, 1))
+    g, v = gpu_build(same)
+    out, cnt, _ = gpu_walk(g, n, eps=0.1, mac_kind=1, mac_param=0.5)
+    assert np.all(out[:, :3] == 0) and np.allclose(out[:, 3], -(n - 1) * 0.5 / 0.1, rtol=1e-5)
+    g.close()
+    # a massless tracer feels the field and sources nothing; a system far from the origin keeps its accuracy relative to eq. 1
+    pos = W.plummer(3000, seed=6)
+    pos[17, 3] = 0.0
+    pos[:, :3] += np.array([1000.0, -2000.0, 500.0], np.float32)
+    g, v = gpu_build(pos, n_leaf=8)
+    ref = oracle.direct(v["pos_m_sorted"], 0.05)
+    out, _, _ = gpu_walk(g, 3000, eps=0.05, mac_kind=1, mac_param=0.0)
+    assert np.all(np.isfinite(out)) and np.abs(out - ref).max() < 1e-4 * np.abs(ref).max()
+    out, cnt, _ = gpu_walk(g, 3000, eps=0.05, mac_kind=1, mac_param=0.6, r_crit=0.5)
+    refw, c = _oracle_on_gpu_tree(oracle, v, eps=0.05, mac_kind=1, mac_param=0.6, r_crit=0.5)
+    assert cnt == c["interactions"]
+    _assert_parity(out, refw, np.arange(3000))
+    g.close()
