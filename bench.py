@@ -43,7 +43,7 @@ FLOP_PER_INTERACTION = 24          # 20 + rsqrt counted as 4 (the paper's GTX TI
 THETA_BOOTSTRAP = 0.5              # DESIGN.md R7
 # dram__bytes_read.sum + dram__bytes_write.sum per k_walk launch, mean over the 8 substep launches of one cycle of the default
 # workload, from the ncu capture summarised in profiles/r01_walk_traffic.md (a profiler number: quoted, never measured here)
-NCU_WALK_TRAFFIC_BYTES = {"nfw_2p24_block": 364649344}
+NCU_WALK_TRAFFIC_BYTES = {"nfw_2p24_block": 366973024}
 ETA, MAX_LEVELS = 0.5, 8           # BASELINE.json configs[2]
 
 
