@@ -296,3 +296,37 @@ def test_walk_edge_cases(oracle):
     assert cnt == c["interactions"]
     _assert_parity(out, refw, np.arange(3000))
     g.close()
+
+
+def test_walk_randomised_parity_sweep(oracle):
+    """24 seeded draws over model, n, G, n_leaf, eps, active fraction, r_crit, ball, MAC and accuracy parameter (some with a clump of
+    coincident particles: a level-21 leaf wider than one pop): interaction counts equal the oracle's, forces within tolerance."""
+    from gpu_util import gpu_build, gpu_walk, acc_rel_err
+    rng = np.random.default_rng(123)
+    for it in range(24):
+        model = ["plummer", "hernquist", "nfw", "m31_like"][it % 4]
+        n = int(rng.integers(2000, 60000))
+        G = [32, 16, 8][it % 3]
+        n_leaf = int(rng.choice([1, 4, 8, 16, 32, 64]))
+        pos = getattr(W, model)(n, seed=100 + it)
+        if it % 5 == 0:
+            k = int(rng.integers(100, 700))
+            j = int(rng.integers(0, n - k))
+            pos[j:j + k, :3] = pos[j, :3]
+        eps = float(2.0 ** -rng.integers(5, 10))
+        g, v = gpu_build(pos, n_leaf=n_leaf, group_size=G)
+        _, _, aold = gpu_walk(g, n, eps=eps, mac_kind=1, mac_param=0.5, amag=True, count=False)
+        frac = float(rng.choice([1.0, 1.0, 0.5, 0.05, 0.005]))
+        active = None if frac == 1.0 else W.random_active_subset(n, frac, seed=it)
+        rows = np.arange(n) if active is None else active
+        r_crit = float(rng.choice([np.inf, 1.0, 0.3, 0.05, 0.0]))
+        ball = int(rng.integers(0, 2))
+        g.set_ball(ball)
+        kind = int(rng.integers(0, 3))
+        param = {0: 2.0 ** -float(rng.integers(4, 18)), 1: float(rng.uniform(0.15, 0.9)), 2: 2.0 ** -float(rng.integers(0, 16))}[kind]
+        out, cnt, _ = gpu_walk(g, n, eps=eps, mac_kind=kind, mac_param=param, aold=aold, active=active, r_crit=r_crit)
+        ref, c = _oracle_on_gpu_tree(oracle, v, eps=eps, mac_kind=kind, mac_param=param, aold=aold, active=active, group_size=G,
+                                     r_crit=r_crit, ball_kind=ball, B2=v["node_b2"])
+        assert cnt == c["interactions"], (it, model, n, G, n_leaf, frac, r_crit, ball, kind, param)
+        _assert_parity(out, ref, rows)
+        g.close()
