@@ -375,8 +375,34 @@ static inline float dist2f(const float *a, const float *b)
  *     ties) spans the first sphere: centre = midpoint, radius = distance from the centre to the pair's maximum point.  Pass 2,
  *     members in ascending order: a point at distance dist > r grows the sphere just enough to contain it and the old sphere:
  *     r' = (r + dist)/2, centre moves by (dist - r')/dist of the way to the point.  fp32, operations as written (R17). */
+static float ball_radius2(const float *pos_sorted, const uint32_t *members, uint32_t k, const float rI[3])
+{
+    float b2max = 0.0f;
+    for (uint32_t q = 0; q < k; q++) b2max = std::max(b2max, dist2f(pos_sorted + 4 * (size_t)members[q], rI));
+    return b2max;
+}
+
+/*   ball_kind 2, COM (item 4): centre of mass of the members, sums over the members in ascending order with one fmaf each, then
+ *     one division per coordinate.
+ *   ball_kind 3, CMP (item 5): the smaller of the GEO and COM balls (GEO on ties). */
 static void ball_centre(const float *pos_sorted, const uint32_t *members, uint32_t k, int ball_kind, float rI[3])
 {
+    if (ball_kind == 2 || ball_kind == 3) {
+        float sx = 0.0f, sy = 0.0f, sz = 0.0f, sm = 0.0f;
+        for (uint32_t q = 0; q < k; q++) {
+            const float *p = pos_sorted + 4 * (size_t)members[q];
+            sx = fmaf(p[3], p[0], sx); sy = fmaf(p[3], p[1], sy); sz = fmaf(p[3], p[2], sz); sm += p[3];
+        }
+        float com[3] = {sx / sm, sy / sm, sz / sm};
+        if (!(sm > 0.0f)) ball_centre(pos_sorted, members, k, 0, com);          /* massless members: fall back to GEO */
+        if (ball_kind == 3) {
+            float geo[3];
+            ball_centre(pos_sorted, members, k, 0, geo);
+            if (ball_radius2(pos_sorted, members, k, geo) <= ball_radius2(pos_sorted, members, k, com)) { com[0] = geo[0]; com[1] = geo[1]; com[2] = geo[2]; }
+        }
+        rI[0] = com[0]; rI[1] = com[1]; rI[2] = com[2];
+        return;
+    }
     if (ball_kind == 0) {
         float lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
         for (uint32_t q = 0; q < k; q++)
@@ -433,7 +459,7 @@ void oracle_walk(const float *pos_sorted, uint32_t n,
                  const float *com4, const float *bJ, const float *B2 /* eq. 4; needed iff mac_kind == 2 */,
                  const uint32_t *active, uint32_t n_active, int G,
                  float eps, int mac_kind, float mac_param, const float *aold,
-                 uint32_t group_lo, uint32_t group_hi, float r_crit, int ball_kind /* 0 GEO, 1 EBS (App. B) */,
+                 uint32_t group_lo, uint32_t group_hi, float r_crit, int ball_kind /* 0 GEO, 1 EBS, 2 COM, 3 CMP (App. B) */,
                  double *out4, uint64_t *counts)
 {
     const uint32_t n_groups = (n + (uint32_t)G - 1) / (uint32_t)G;

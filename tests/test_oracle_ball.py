@@ -25,7 +25,7 @@ def _seb_radius(x, iters=4000):
 def test_members_are_enclosed_and_radius_is_the_exact_maximum():
     rng = np.random.default_rng(1)
     for k in (1, 2, 3, 5, 17, 32):
-        for kind in (0, 1):
+        for kind in (0, 1, 2, 3):
             p = _pts(k, rng, scale=10.0 ** rng.uniform(-3, 1))
             ball = oracle.group_ball(p, np.arange(k), kind)
             d = np.sqrt(((p[:, :3].astype(np.float64) - ball[:3].astype(np.float64)) ** 2).sum(1))
@@ -38,7 +38,7 @@ def test_special_cases():
     two = np.array([[0, 0, 0, 1], [2, 4, 4, 1]], np.float32)                       # distance 6
     line = np.zeros((9, 4), np.float32)
     line[:, 0] = np.arange(9)                                                      # collinear: diameter 8
-    for kind in (0, 1):
+    for kind in (0, 1, 2, 3):
         b = oracle.group_ball(one, [0], kind)
         assert np.array_equal(b[:3], one[0, :3]) and b[3] == 0
         b = oracle.group_ball(two, [0, 1], kind)
@@ -49,7 +49,7 @@ def test_special_cases():
     rng = np.random.default_rng(2)
     p = _pts(40, rng)
     mem = np.array([3, 7, 8, 20, 31], np.uint32)
-    for kind in (0, 1):
+    for kind in (0, 1, 2, 3):
         assert np.array_equal(oracle.group_ball(p, mem, kind), oracle.group_ball(p[mem], np.arange(5), kind))
 
 
@@ -67,3 +67,26 @@ def test_radii_against_the_smallest_enclosing_ball():
     assert geo.min() > 1 - 2e-3 and ebs.min() > 1 - 2e-3               # nothing beats the smallest ball (iteration tolerance)
     assert np.median(ebs) < 1.08 and ebs.max() < 1.25
     assert np.median(geo) < 1.15 and np.median(ebs) < np.median(geo)   # EBS is the tighter of the two (Fig. B.10)
+
+
+def test_com_and_cmp_balls():
+    """App. B items 4 and 5: COM is centred on the mass-weighted mean of the members; CMP is the smaller of GEO and COM; COM is the
+    loosest of the generators ("r_ball in the COM is much bigger")."""
+    rng = np.random.default_rng(7)
+    r = {0: [], 2: [], 3: []}
+    for _ in range(200):
+        k = int(rng.integers(2, 33))
+        p = _pts(k, rng)
+        p[:, 3] = rng.uniform(0.1, 3.0, k).astype(np.float32)
+        com = (p[:, 3:4].astype(np.float64) * p[:, :3]).sum(0) / p[:, 3].astype(np.float64).sum()
+        b = {kind: oracle.group_ball(p, np.arange(k), kind) for kind in (0, 2, 3)}
+        assert np.allclose(b[2][:3], com, atol=2e-6 * np.abs(p[:, :3]).max())
+        assert b[3][3] == min(b[0][3], b[2][3])
+        assert np.array_equal(b[3], b[0]) or np.array_equal(b[3], b[2])
+        for kind in r:
+            r[kind].append(b[kind][3])
+    assert np.mean(r[2]) > np.mean(r[0]) >= np.mean(r[3])
+    # massless members: COM is undefined, the ball falls back to GEO
+    p = _pts(6, rng)
+    p[:, 3] = 0.0
+    assert np.array_equal(oracle.group_ball(p, np.arange(6), 2), oracle.group_ball(p, np.arange(6), 0))
