@@ -41,7 +41,7 @@ enum {
 };
 
 enum { GOTHIC_KEY_PEANO_HILBERT = 0, GOTHIC_KEY_MORTON = 1 };   /* PAPER.md:54 / PAPER.md:564 */
-enum { GOTHIC_BALL_GEO = 0, GOTHIC_BALL_EBS = 1 };                  /* enclosing ball of an i-group, App. B PAPER.md:568 items 3 and 2 */
+enum { GOTHIC_BALL_GEO = 0, GOTHIC_BALL_EBS = 1, GOTHIC_BALL_COM = 2, GOTHIC_BALL_CMP = 3 };   /* enclosing ball of an i-group, App. B PAPER.md:568 items 3, 2, 4, 5 */
 enum { GOTHIC_MAC_ACCELERATION = 0, GOTHIC_MAC_OPENING_ANGLE = 1, GOTHIC_MAC_MULTIPOLE = 2 }; /* eq. 5 PAPER.md:85-89 / eq. 2 PAPER.md:68-72 / eq. 3-4 */
 
 /* Allocates a context for up to n_max particles.
@@ -159,7 +159,8 @@ int gothic_block_cycle_host(gothic_ctx *ctx, const float *pos_m_host, const floa
                             uint8_t *level_host, int32_t *info_host, unsigned long long *n_interactions_host, void *stream);
 
 /* Enclosing ball of the pseudo i-particle used by the following walks (App. B): GOTHIC_BALL_GEO (default;
- * centre of the members' bounding cuboid) or GOTHIC_BALL_EBS (Ritter's efficient bounding sphere; R17).  In both the
+ * centre of the members' bounding cuboid), GOTHIC_BALL_EBS (Ritter's efficient bounding sphere; R17), GOTHIC_BALL_COM
+ * (centre of mass of the members) or GOTHIC_BALL_CMP (the smaller of GEO and COM).  In all of them the
  * radius is the exact maximum distance of the members from the centre.  Also decides the r_crit splitting (R13). */
 int gothic_set_ball(gothic_ctx *ctx, int ball_kind);
 

@@ -35,7 +35,7 @@ def test_balls_study(capsys):
     from paper_1610_07279_b200 import studies
     studies.study_balls(1 << 15)
     rows = _lines(capsys)
-    assert len(rows) == 24
+    assert len(rows) == 48          # 4 balls x 3 MACs x 4 parameters
     for mac in ("acceleration", "multipole", "opening_angle"):
         geo = [d for d in rows if d["ball"] == "GEO" and d["mac"] == mac]
         assert all(b["err_median"] < a["err_median"] and b["interactions"] > a["interactions"] for a, b in zip(geo, geo[1:]))
