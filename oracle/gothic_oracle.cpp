@@ -20,7 +20,10 @@
  *   tree                  : independent recursive builder + partition invariants
  *   moments               : numpy brute force (P:62 definitions)
  *   walk                  : Delta=0 equals eq. 1; error shrinks as Delta tightens;
- *                           Plummer closed form at large N; momentum
+ *                           Plummer closed form at large N; momentum;
+ *                           eq. 5 / eq. 2 / eq. 3 written literally in pure-Python per-particle walks (r_crit = 0);
+ *                           group a_min = min over members (R4): pure-Python group walk with |a_old| spread over four
+ *                           decades + "group acceptance => eq. 5 holds for every member"
  *   levels / active set   : closed-form NFW level fractions; nesting invariants
  * Parity UNPINNED (report only): absolute error-vs-Delta values and interactions per step (the paper
  * gives them only as figures).

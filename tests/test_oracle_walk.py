@@ -260,3 +260,96 @@ def test_rcrit_zero_is_the_textbook_per_particle_tree_walk(oracle):
                 n_int += 1
     assert c["groups"] == n and c["interactions"] == n_int
     assert np.allclose(out, ref, rtol=1e-11, atol=1e-13)
+
+
+# ---- pins for the group's a_min (reading R4) and for the opening-angle criterion (eq. 2) -------------------
+def _fma32(a, b, c):
+    """fmaf on float32 values: the product of two float32 is exact in double; one rounding to float32 of the sum."""
+    return np.float32(np.float64(a) * np.float64(b) + np.float64(c))
+
+
+def _python_group_walk(t, members, ball, thr, accept_fn, eps):
+    """O7 for one piece, written out: pending stack from the root, eq. 6-7 distance to the ball surface in fp32, the caller's
+    acceptance test, monopole sums in double.  Returns (accepted cells, particle entries, out[k,4], MAC tests)."""
+    f32, P = np.float32, t.pos_sorted
+    eps2 = float(f32(eps)) ** 2
+    cells, parts, tests = [], [], 0
+    stack = [0]
+    while stack:
+        J = stack.pop()
+        tests += 1
+        d3 = (t.com[J, :3] - ball[:3]).astype(f32)
+        r2 = _fma32(d3[2], d3[2], _fma32(d3[1], d3[1], f32(d3[0] * d3[0])))
+        d = max(f32(f32(np.sqrt(r2)) - ball[3]), f32(0.0))          # eq. 6-7: distance to the nearest point of the ball
+        if d > 0 and accept_fn(J, d):
+            cells.append(J)
+        elif t.child[J] == 0xFFFFFFFF:
+            parts.extend(range(t.head[J], t.head[J] + t.num[J]))
+        else:
+            stack.extend(range(t.child[J], t.child[J] + t.nchild[J]))
+    out = np.zeros((len(members), 4))
+    for q, i in enumerate(members):
+        src = [t.com[J].astype(np.float64) for J in cells] + [P[s].astype(np.float64) for s in parts if s != i]
+        for e in src:
+            dx = e[:3] - P[i, :3].astype(np.float64)
+            u = 1.0 / np.sqrt(dx @ dx + eps2)
+            out[q, :3] += e[3] * u ** 3 * dx
+            out[q, 3] -= e[3] * u
+    return cells, parts, out, tests
+
+
+@pytest.mark.parametrize("G", [8, 32])
+def test_group_amin_is_the_minimum_over_members(oracle, G):
+    """Reading R4 + P:118 ("conservative"): a group tests eq. 5 with Delta_acc * min_k |a_old,k| and the distance from the ball
+    surface, so that a cell accepted for the group is accepted by eq. 5 for EVERY member with that member's own
+    |a_old| and own distance.  |a_old| is spread over four decades inside every group, so a max, a mean or 'first member'
+    reading changes the lists.  Value pin: a pure-Python group walk with thr = Delta * min(aold[K]) reproduces the oracle's
+    counts and sums; property pin: group acceptance => per-particle acceptance, evaluated in double."""
+    n = 400
+    pos = W.plummer(n, seed=21)
+    t = oracle.build_tree(pos, n_leaf=4)
+    eps, dacc = 0.02, 2.0 ** -5
+    rng = np.random.default_rng(5)
+    aold = (10.0 ** rng.uniform(-2.0, 2.0, n)).astype(np.float32)          # four decades, uncorrelated with position
+    out, c = oracle.walk_tree(t, eps=eps, mac_kind=0, mac_param=dacc, aold=aold, group_size=G)
+    f32 = np.float32
+    n_int = n_tests = n_list = n_checked = 0
+    p64 = t.pos_sorted.astype(np.float64)
+    for g in range((n + G - 1) // G):
+        K = np.arange(g * G, min(n, (g + 1) * G), dtype=np.uint32)
+        ball = oracle.group_ball(t.pos_sorted, K)
+        thr = f32(f32(dacc) * aold[K].min())
+        mb2 = lambda J: f32(f32(t.com[J, 3] * t.b[J]) * t.b[J])
+        cells, parts, ref, tests = _python_group_walk(
+            t, K, ball, thr, lambda J, d: f32(thr * f32(f32(d * d) * f32(d * d))) >= mb2(J), eps)
+        assert np.allclose(out[K], ref, rtol=1e-11, atol=1e-13)
+        n_int += len(K) * (len(cells) + len(parts)); n_tests += tests; n_list += len(cells) + len(parts)
+        for J in cells:                 # eq. 5 per member: Delta |a_i| d_i^4 >= m_J b_J^2, all in double
+            di = np.linalg.norm(p64[K, :3] - t.com[J, :3].astype(np.float64), axis=1)
+            lhs = dacc * aold[K].astype(np.float64) * di ** 4
+            assert np.all(lhs >= float(t.com[J, 3]) * float(t.b[J]) ** 2 * (1 - 1e-5))
+            n_checked += 1
+    assert c["interactions"] == n_int and c["mac_tests"] == n_tests and c["list_entries"] == n_list
+    assert n_checked > 10 * (n // G)        # the pin is not vacuous: cells are accepted
+
+
+def test_opening_angle_is_b_over_d(oracle):
+    """eq. 2: a cell is accepted when b_J / d <= theta, b_J the RADIUS of the cell's sphere and d the distance
+    to it.  r_crit = 0 makes every particle its own group (b_I = 0, d = |r_J - r_i|): the textbook per-particle walk, the
+    criterion written literally in double.  Counts and sums must equal the oracle's (a diameter-for-radius slip, or d^2 for
+    d, changes the lists)."""
+    n = 400
+    pos = W.hernquist(n, seed=14)
+    t = oracle.build_tree(pos, n_leaf=4)
+    eps, theta = 0.02, 0.6
+    out, c = oracle.walk_tree(t, eps=eps, mac_kind=1, mac_param=theta, r_crit=0.0)
+    n_int = n_tests = n_cells = 0
+    theta32 = float(np.float32(theta))
+    for i in range(n):
+        K = np.array([i], np.uint32)
+        ball = np.append(t.pos_sorted[i, :3], np.float32(0.0)).astype(np.float32)
+        cells, parts, ref, tests = _python_group_walk(t, K, ball, None, lambda J, d: float(t.b[J]) / float(d) <= theta32, eps)
+        assert np.allclose(out[i], ref[0], rtol=1e-11, atol=1e-13)
+        n_int += len(cells) + len(parts); n_tests += tests; n_cells += len(cells)
+    assert c["groups"] == n and c["interactions"] == n_int and c["mac_tests"] == n_tests
+    assert n_cells > 20 * n         # cells are accepted: the criterion is exercised
