@@ -19,8 +19,13 @@ Interactions are counted in a separate, identical, untimed replay ("in a 
 N > 1 (torchrun): the path is single-GPU by design (BASELINE.json north_star: "one GPU only"), so every rank runs an
 independent replica (its own seed); no data-path collective; time = max over ranks; value = sum of interactions / time.
 
+After the headline workload, rank 0 of an N = 1 run also times the other BASELINE.json configs (m31_2p24_block, hernquist_2p20,
+plummer_2p13 and a reduced grid of the nfw_2p22_sweep: Delta_acc x active fraction) with a few steps each and reports them
+under "other_configs" (walk ms, interactions, interactions/s, fraction of the FP32 peak at 24 flop, ms per block step);
+--headline-only skips them.
+
 --impl reference: times the CPU oracle (oracle/, as it stands) on the host cores on a bounded sample of the same
-workload; rank 0 only.
+workload (the walks of every substep of one block cycle on a sample of i-groups; build, levels, moments untimed); rank 0 only.
 """
 from __future__ import annotations
 
@@ -41,10 +46,24 @@ METRIC = "tree_walk_interactions_per_s_block_cycle"
 UNIT = "interactions/s"
 FLOP_PER_INTERACTION = 24          # 20 + rsqrt counted as 4 (the paper's GTX TITAN X convention); 20 and 28 also reported
 THETA_BOOTSTRAP = 0.5              # DESIGN.md R7
-# dram__bytes_read.sum + dram__bytes_write.sum per k_walk launch, mean over the 8 substep launches of one cycle of the default
-# workload, from the ncu capture summarised in profiles/r01_walk_traffic.md (a profiler number: quoted, never measured here)
-NCU_WALK_TRAFFIC_BYTES = {"nfw_2p24_block": 366973024}
+# dram__bytes_read.sum + dram__bytes_write.sum per k_walk launch (mean over the substep launches of one cycle) is a profiler
+# number: it is read from the tracked summary below (which names the commit and the command it was measured with), never
+# measured here; null when the file has no entry for the workload
+WALK_TRAFFIC_FILE = os.path.join(ROOT, "profiles", "walk_traffic.json")
+OTHER_CONFIGS = ["m31_2p24_block", "hernquist_2p20", "plummer_2p13"]
+SWEEP_LOG2_DELTA = [1, 5, 9, 13, 20]       # reduced grid of BASELINE.json configs[4]
+SWEEP_ACTIVE = [0.01, 0.10, 1.00]
 ETA, MAX_LEVELS = 0.5, 8           # BASELINE.json configs[2]
+
+
+def _walk_traffic(workload: str):
+    try:
+        with open(WALK_TRAFFIC_FILE) as f:
+            d = json.load(f)
+        e = d["workloads"].get(workload)
+        return (e["bytes_per_launch"], f"profiles/walk_traffic.json (ncu, commit {d['commit']})") if e else (None, None)
+    except Exception:
+        return None, None
 
 
 def _peaks() -> dict:
@@ -68,7 +87,7 @@ class ClockSampler:
             import pynvml
             pynvml.nvmlInit()
             self._nv = pynvml
-            self._h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(index or 0)
             self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
         except Exception:
             self._nv = None
@@ -107,54 +126,8 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------------------------
-def run_reference(args, rank: int, world: int):
-    """The CPU oracle, as it stands, on the host cores: a bounded sample of the workload's all-active substep."""
-    if rank != 0:
-        return
-    import oracle
-    from paper_1610_07279_b200 import workloads as W
-    t0 = time.time()
-    pos, cfg = W.make_config(args.workload, seed=args.seed, n=args.n)
-    n, eps, dacc = cfg["n"], cfg["eps"], cfg["delta_acc"]
-    r_crit = cfg["r_crit"] if args.r_crit is None else args.r_crit
-    t_gen = time.time() - t0
-    t0 = time.time()
-    tree = oracle.build_tree(pos)
-    t_build = time.time() - t0
-    G = 32
-    n_groups = (n + G - 1) // G
-    cores = oracle.num_threads()
-    ranges = _sample_ranges(n_groups, args.ref_groups, 8)
-    # |a_old| for the sample: the oracle's own opening-angle bootstrap on the same groups (DESIGN.md R7)
-    aold = np.ones(n, np.float32)
-    for lo, hi in ranges:
-        o, _ = oracle.walk_tree(tree, eps=eps, mac_kind=1, mac_param=THETA_BOOTSTRAP, group_range=(lo, hi))
-        aold[lo * G:hi * G] = np.linalg.norm(o[lo * G:hi * G, :3], axis=1).astype(np.float32)
-
-    def step():
-        cnt = 0
-        for lo, hi in ranges:
-            _, c = oracle.walk_tree(tree, eps=eps, mac_kind=0, mac_param=dacc, aold=aold, group_range=(lo, hi), r_crit=r_crit)
-            cnt += c["interactions"]
-        return cnt
-
-    for _ in range(args.warmup):
-        step()
-    t0 = time.time()
-    inter = 0
-    for _ in range(args.steps):
-        inter += step()
-    dt = time.time() - t0
-    val = inter / dt
-    sample = (f"{sum(hi - lo for lo, hi in ranges)} of {n_groups} i-groups (8 evenly spaced runs) of the all-active substep, "
-              f"fp64 accumulation, {inter // args.steps} interactions per step; oracle tree build {t_build:.1f} s (untimed)")
-    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-            "data": "synthetic", "config": {"workload": args.workload, "n": n, "eps": eps, "delta_acc": dacc, "r_crit": r_crit, "seed": args.seed},
-            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
-            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-            "gpu_launches": 0, "setup_s": {"generate": t_gen, "oracle_build": t_build}}
-    print(json.dumps(line), flush=True)
+REFERENCE_SCOPE = ("the walks (W1-W6) of every substep of one block cycle on a sample of i-groups, fp64 accumulation; the oracle's tree build, "
+                   "levels, active lists and moments are not in the timed region (the GPU arm's cycle includes them); not like for like")
 
 
 def _sample_ranges(n_groups: int, want: int, pieces: int):
@@ -170,38 +143,104 @@ def _sample_ranges(n_groups: int, want: int, pieces: int):
     return out
 
 
-def cpu_baseline(pos, cfg, r_crit: float, budget_s: float = 15.0) -> dict:
-    """Oracle walk (fp64 sum, OpenMP over groups) on a sample of the all-active substep sized to ~budget_s."""
-    import oracle
+def oracle_cycle_sample(oracle, tree, cfg, r_crit: float, ranges, G: int = 32):
+    """The oracle's share of one step on the sampled i-groups: |a_old| from its own opening-angle bootstrap (R7), block
+    levels of the sampled particles (oracle.levels), then step() = the acceleration-MAC walk of every substep's active set.
+    Returns (step, n_substeps); step() returns the interactions it evaluated."""
     n, eps, dacc = cfg["n"], cfg["eps"], cfg["delta_acc"]
+    aold = np.ones(n, np.float32)
+    acc = np.zeros((n, 4), np.float32)
+    for lo, hi in ranges:
+        o, _ = oracle.walk_tree(tree, eps=eps, mac_kind=1, mac_param=THETA_BOOTSTRAP, group_range=(lo, hi))
+        acc[lo * G:hi * G] = o[lo * G:hi * G]
+        aold[lo * G:hi * G] = np.linalg.norm(o[lo * G:hi * G, :3], axis=1).astype(np.float32)
+    actives = [None]
+    if cfg["block"]:
+        sel = np.concatenate([np.arange(lo * G, min(n, hi * G), dtype=np.uint32) for lo, hi in ranges])
+        lev, _, n_lev = oracle.levels(acc[sel], eps, ETA, MAX_LEVELS)
+        actives = []
+        for s in range(1, (1 << (n_lev - 1)) + 1):
+            ctz = (s & -s).bit_length() - 1
+            actives.append(np.ascontiguousarray(sel[lev <= ctz]))
+
+    def step():
+        cnt = 0
+        for act in actives:
+            if act is not None and act.size == 0:
+                continue
+            for lo, hi in ranges:
+                _, c = oracle.walk_tree(tree, eps=eps, mac_kind=0, mac_param=dacc, aold=aold, active=act, group_range=(lo, hi), r_crit=r_crit)
+                cnt += c["interactions"]
+        return cnt
+    return step, len(actives)
+
+
+def run_reference(args, rank: int, world: int):
+    """The CPU oracle, as it stands, on the host cores: a bounded sample of the workload's block cycle."""
+    if rank != 0:
+        return
+    import oracle
+    from paper_1610_07279_b200 import workloads as W
+    t0 = time.time()
+    pos, cfg = W.make_config(args.workload, seed=args.seed, n=args.n)
+    n, eps, dacc = cfg["n"], cfg["eps"], cfg["delta_acc"]
+    r_crit = cfg["r_crit"] if args.r_crit is None else args.r_crit
+    t_gen = time.time() - t0
     t0 = time.time()
     tree = oracle.build_tree(pos)
     t_build = time.time() - t0
-    G = 32
-    n_groups = (n + G - 1) // G
+    n_groups = (n + 31) // 32
+    cores = oracle.num_threads()
+    ranges = _sample_ranges(n_groups, args.ref_groups, 8)
+    step, n_sub = oracle_cycle_sample(oracle, tree, cfg, r_crit, ranges)
+    for _ in range(args.warmup):
+        step()
+    t0 = time.time()
+    inter = 0
+    for _ in range(args.steps):
+        inter += step()
+    dt = time.time() - t0
+    val = inter / dt
+    sample = (f"{sum(hi - lo for lo, hi in ranges)} of {n_groups} i-groups (8 evenly spaced runs), all {n_sub} substeps of the block cycle, "
+              f"fp64 accumulation, {inter // max(args.steps, 1)} interactions per step; oracle tree build {t_build:.1f} s (untimed)")
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": 1e3 * dt / max(args.steps, 1), "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": {"workload": args.workload, "n": n, "eps": eps, "delta_acc": dacc, "r_crit": r_crit, "seed": args.seed},
+            "reference_scope": REFERENCE_SCOPE,
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0, "setup_s": {"generate": t_gen, "oracle_build": t_build}}
+    print(json.dumps(line), flush=True)
+
+
+def cpu_baseline(pos, cfg, r_crit: float, budget_s: float = 15.0) -> dict:
+    """Oracle walks (fp64 sum, OpenMP over groups) of one block cycle on a sample of i-groups sized to ~budget_s."""
+    import oracle
+    n = cfg["n"]
+    t0 = time.time()
+    tree = oracle.build_tree(pos)
+    t_build = time.time() - t0
+    n_groups = (n + 31) // 32
     cores = oracle.num_threads()
 
     def run(ranges):
-        aold = np.ones(n, np.float32)
-        for lo, hi in ranges:
-            o, _ = oracle.walk_tree(tree, eps=eps, mac_kind=1, mac_param=THETA_BOOTSTRAP, group_range=(lo, hi))
-            aold[lo * G:hi * G] = np.linalg.norm(o[lo * G:hi * G, :3], axis=1).astype(np.float32)
+        step, n_sub = oracle_cycle_sample(oracle, tree, cfg, r_crit, ranges)
         t0 = time.time()
-        cnt = 0
-        for lo, hi in ranges:
-            _, c = oracle.walk_tree(tree, eps=eps, mac_kind=0, mac_param=dacc, aold=aold, group_range=(lo, hi), r_crit=r_crit)
-            cnt += c["interactions"]
-        return cnt, time.time() - t0
+        cnt = step()
+        return cnt, time.time() - t0, n_sub
 
     probe = _sample_ranges(n_groups, 64 * cores, 8)
-    cnt, dt = run(probe)
-    want = int(sum(hi - lo for lo, hi in probe) * (budget_s / 2.2) / max(dt, 1e-3))   # bootstrap + MAC walk ~ 2.2 x the timed part
+    t0 = time.time()
+    cnt, dt, n_sub = run(probe)
+    t_probe = time.time() - t0          # bootstrap + levels + timed walks
+    want = int(sum(hi - lo for lo, hi in probe) * budget_s / max(t_probe, 1e-3))
     ranges = _sample_ranges(n_groups, want, 8)
-    cnt, dt = run(ranges)
+    cnt, dt, n_sub = run(ranges)
     ng = sum(hi - lo for lo, hi in ranges)
     return {"value": cnt / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": f"{ng} of {n_groups} i-groups (8 evenly spaced runs) of the all-active substep, fp64 accumulation, {cnt} interactions in "
-                      f"{dt:.2f} s; oracle tree build at full N took {t_build:.1f} s (not in the rate)"}
+            "sample": f"{ng} of {n_groups} i-groups (8 evenly spaced runs), all {n_sub} substeps of the block cycle, fp64 accumulation, {cnt} interactions in "
+                      f"{dt:.2f} s; oracle tree build at full N took {t_build:.1f} s (not in the rate)",
+            "scope": REFERENCE_SCOPE}
 
 
 # ------------------------------------------------------------------------------------------------------------
@@ -217,26 +256,15 @@ def aggregate_over_ranks(dist, times_ms, counts, device):
     return [float(x) for x in t_all.tolist()], [int(x) for x in i_all.tolist()]
 
 
-def run_ours(args, rank: int, world: int, local_rank: int):
-    import torch
-    from paper_1610_07279_b200 import workloads as W
-    from paper_1610_07279_b200.binding import Gothic, MAC_ACCELERATION, MAC_OPENING_ANGLE
-
-    torch.cuda.set_device(local_rank)
-    dev = torch.device("cuda", local_rank)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=dev)
-
-    peaks = _peaks()
-    pos_np, cfg = W.make_config(args.workload, seed=args.seed + rank, n=args.n)
+def measure_cycle(torch, W, B, workload: str, *, seed: int, n, r_crit, steps: int, warmup: int, dev, barrier, clock_index=None, with_e2e: bool = True):
+    """Times `steps` block cycles of one workload on the current device (after `warmup` untimed ones) and replays them untimed with
+    the interaction counter on.  Returns a dict of raw measurements of this rank."""
+    pos_np, cfg = W.make_config(workload, seed=seed, n=n)
     n, eps, dacc = cfg["n"], cfg["eps"], cfg["delta_acc"]
-    block = cfg["block"]
-    r_crit = cfg["r_crit"] if args.r_crit is None else args.r_crit
-    props = torch.cuda.get_device_properties(dev)
+    block, G = cfg["block"], cfg["group_size"]
+    r_crit = cfg["r_crit"] if r_crit is None else r_crit
 
-    g = Gothic(n)
+    g = B.Gothic(n, group_size=G)
     pos_host = torch.from_numpy(pos_np).pin_memory()
     pos = pos_host.to(dev, non_blocking=True)
     acc = torch.zeros(n, 4, dtype=torch.float32, device=dev)
@@ -245,12 +273,11 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     active = torch.zeros(n, dtype=torch.int32, device=dev)
     n_act = torch.zeros(1, dtype=torch.int32, device=dev)
     emin_nlev = torch.zeros(2, dtype=torch.int32, device=dev)
-    counter = torch.zeros(1, dtype=torch.int64, device=dev)
 
     # ---- untimed bootstrap (R7): opening-angle walk -> |a_old|, then one acceleration-MAC walk -------------
     g.build_tree(pos)
-    g.walk_tree(acc, eps=eps, mac_kind=MAC_OPENING_ANGLE, mac_param=THETA_BOOTSTRAP, amag_out=amag, r_crit=r_crit)
-    g.walk_tree(acc, eps=eps, mac_kind=MAC_ACCELERATION, mac_param=dacc, aold=amag, amag_out=amag, r_crit=r_crit)
+    g.walk_tree(acc, eps=eps, mac_kind=B.MAC_OPENING_ANGLE, mac_param=THETA_BOOTSTRAP, amag_out=amag, r_crit=r_crit)
+    g.walk_tree(acc, eps=eps, mac_kind=B.MAC_ACCELERATION, mac_param=dacc, aold=amag, amag_out=amag, r_crit=r_crit)
     if block:
         g.set_timesteps(level, acc_pot=acc, eps=eps, eta=ETA, max_levels=MAX_LEVELS, emin_nlev_dev=emin_nlev)
         g.check()
@@ -279,22 +306,16 @@ def run_ours(args, rank: int, world: int, local_rank: int):
             if block:
                 timed("active", lambda: g.set_timesteps(level, acc_pot=None, eps=eps, substep=s, active=active, n_active_dev=n_act))
                 timed("moments", lambda: g.update_moments())
-                timed("walk", lambda: g.walk_tree(acc, eps=eps, mac_kind=MAC_ACCELERATION, mac_param=dacc, aold=amag, active=active,
+                timed("walk", lambda: g.walk_tree(acc, eps=eps, mac_kind=B.MAC_ACCELERATION, mac_param=dacc, aold=amag, active=active,
                                                    n_active_dev=n_act, amag_out=amag, r_crit=r_crit,
                                                    n_interactions=None if counts is None else counts[s - 1:s]))
             else:
-                timed("walk", lambda: g.walk_tree(acc, eps=eps, mac_kind=MAC_ACCELERATION, mac_param=dacc, aold=amag, amag_out=amag, r_crit=r_crit,
+                timed("walk", lambda: g.walk_tree(acc, eps=eps, mac_kind=B.MAC_ACCELERATION, mac_param=dacc, aold=amag, amag_out=amag, r_crit=r_crit,
                                                    n_interactions=None if counts is None else counts[s - 1:s]))
 
-    def barrier():
-        torch.cuda.synchronize()
-        if dist is not None:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    for _ in range(args.warmup):
+    for _ in range(warmup):
         cycle()
-    g.check()
+        g.check()       # the traversal-stack flag is sticky: one check validates every walk of the cycle
     snap = (acc.clone(), amag.clone(), level.clone())
 
     # ---- timed region: exactly K steps -------------------------------------------------------------------------------
@@ -302,15 +323,17 @@ def run_ours(args, rank: int, world: int, local_rank: int):
     ev = []
     t_start, t_stop = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
-    with ClockSampler(local_rank) as clk:
+    with ClockSampler(clock_index) as clk:
         t_start.record()
-        for _ in range(args.steps):
+        for _ in range(steps):
             cycle(ev)
         t_stop.record()
         barrier()
     total_ms = t_start.elapsed_time(t_stop)
     launches = g.launch_count() - launches0
     g.check()
+    if block:
+        assert int(emin_nlev[1].item()) == n_levels, "the number of block levels changed between cycles"
     stage_ms = {k: 0.0 for k in stage_names}
     walk_ms_sub = np.zeros(n_sub)
     wi = 0
@@ -320,16 +343,16 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         if name == "walk":
             walk_ms_sub[wi % n_sub] += ms
             wi += 1
-    walk_launches = wi
 
     # ---- identical untimed replay with the interaction counter on ----------------------------------------------
     acc.copy_(snap[0]); amag.copy_(snap[1]); level.copy_(snap[2])
     counts = torch.zeros(n_sub, dtype=torch.int64, device=dev)
     act_counts = np.zeros(n_sub, np.int64)
     inter_sub = np.zeros(n_sub, np.int64)
-    for _ in range(args.steps):
+    for _ in range(steps):
         counts.zero_()
         cycle(None, counts)
+        g.check()
         inter_sub += counts.cpu().numpy()
     if block:   # active counts per substep (same every cycle: levels are recomputed from converged accelerations)
         for s in range(1, n_sub + 1):
@@ -337,12 +360,11 @@ def run_ours(args, rank: int, world: int, local_rank: int):
             act_counts[s - 1] = int(n_act.item())
     else:
         act_counts[:] = n
-    inter_total = int(inter_sub.sum())
 
     # ---- e2e: same cycle through the host-buffer C-ABI call ---------------------------------------------------------------
     e2e = None
-    if block:
-        k_e2e = max(1, min(args.steps, 3))
+    if with_e2e and block:
+        k_e2e = max(1, min(steps, 3))
         acc_prev_sorted = snap[0]
         perm = g.get_tree_view()["perm"].long()
         acc_prev_orig = torch.empty_like(acc_prev_sorted)
@@ -352,7 +374,8 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         h_out = torch.empty(n, 4, dtype=torch.float32).pin_memory()
         h_lev = torch.empty(n, dtype=torch.uint8).pin_memory()
         del acc_prev_orig, perm
-        g.block_cycle_host(pos_host, h_prev, h_out, eps=eps, delta_acc=dacc, eta=ETA, max_levels=MAX_LEVELS, level_host=h_lev, r_crit=r_crit)   # warm-up
+        kw = dict(eps=eps, delta_acc=dacc, eta=ETA, max_levels=MAX_LEVELS, level_host=h_lev, r_crit=r_crit)
+        g.block_cycle_host(pos_host, h_prev, h_out, **kw)   # warm-up
         h_prev.copy_(h_prev0)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         barrier()
@@ -360,7 +383,7 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         e0.record()
         a, b = h_prev, h_out
         for _ in range(k_e2e):
-            g.block_cycle_host(pos_host, a, b, eps=eps, delta_acc=dacc, eta=ETA, max_levels=MAX_LEVELS, level_host=h_lev, r_crit=r_crit)
+            g.block_cycle_host(pos_host, a, b, **kw)
             a, b = b, a
         e1.record()
         barrier()
@@ -370,10 +393,92 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         h_prev.copy_(h_prev0)
         a, b, e2e_inter = h_prev, h_out, 0
         for _ in range(k_e2e):
-            info = g.block_cycle_host(pos_host, a, b, eps=eps, delta_acc=dacc, eta=ETA, max_levels=MAX_LEVELS, level_host=h_lev, count=True, r_crit=r_crit)
+            info = g.block_cycle_host(pos_host, a, b, count=True, **kw)
             e2e_inter += info["interactions"]
             a, b = b, a
         e2e = {"ms": e2e_ms, "steps": k_e2e, "interactions": e2e_inter, "h2d": 2 * n * 16, "d2h": n * 16 + n}
+    g.close()
+    return {"cfg": cfg, "pos_np": pos_np, "n": n, "r_crit": r_crit, "n_levels": n_levels, "n_sub": n_sub, "steps": steps, "total_ms": total_ms,
+            "stage_ms": stage_ms, "walk_ms_sub": walk_ms_sub, "walk_launches": wi, "inter_sub": inter_sub, "inter_total": int(inter_sub.sum()),
+            "act_counts": act_counts, "launches": int(launches), "e2e": e2e, "clocks": clk.summary()}
+
+
+def summarise(m: dict, alu_peak: float) -> dict:
+    """The per-workload numbers north_star asks for: walk time, interactions/s, TFLOP/s, fraction of the FP32 peak, whole-step time."""
+    K, n_sub = m["steps"], m["n_sub"]
+    walk_rate = m["inter_total"] / (m["stage_ms"]["walk"] * 1e-3)
+    return {"n": m["n"], "r_crit": m["r_crit"], "group_size": m["cfg"]["group_size"], "n_levels": m["n_levels"], "n_substeps": n_sub, "steps": K,
+            "ms_per_cycle": m["total_ms"] / K, "ms_per_block_step": m["total_ms"] / K / n_sub,
+            "interactions_per_cycle": m["inter_total"] // K, "interactions_per_s_cycle": m["inter_total"] / (m["total_ms"] * 1e-3),
+            "walk_ms_per_cycle": m["stage_ms"]["walk"] / K, "walk_interactions_per_s": walk_rate,
+            "walk_tflops_24": walk_rate * 24 / 1e12, "walk_frac_fp32_peak_24": walk_rate * FLOP_PER_INTERACTION / 1e12 / alu_peak,
+            "all_active_walk_ms": m["walk_ms_sub"][-1] / K, "all_active_interactions": int(m["inter_sub"][-1] // K),
+            "stage_ms_per_cycle": {k: v / K for k, v in m["stage_ms"].items()}, "gpu_launches": m["launches"],
+            "e2e_ms_per_cycle": m["e2e"]["ms"] / m["e2e"]["steps"] if m["e2e"] else None, "clocks": m["clocks"]}
+
+
+def measure_sweep(torch, W, B, dev, alu_peak: float, seed: int, reps: int = 3) -> dict:
+    """Reduced grid of BASELINE.json configs[4] on the NFW 2^22 sphere: accuracy parameter x active fraction (random subsets, fixed
+    seed): walk time (best of `reps`, CUDA events), interactions, interactions/s."""
+    pos_np, cfg = W.make_config("nfw_2p22_sweep", seed=seed)
+    n, eps, r_crit = cfg["n"], cfg["eps"], cfg["r_crit"]
+    g = B.Gothic(n, group_size=cfg["group_size"])
+    pos = torch.from_numpy(pos_np).to(dev)
+    acc = torch.zeros(n, 4, dtype=torch.float32, device=dev)
+    amag = torch.zeros(n, dtype=torch.float32, device=dev)
+    cnt = torch.zeros(1, dtype=torch.int64, device=dev)
+    g.build_tree(pos)
+    g.walk_tree(acc, eps=eps, mac_kind=B.MAC_OPENING_ANGLE, mac_param=THETA_BOOTSTRAP, amag_out=amag, r_crit=r_crit)
+    g.walk_tree(acc, eps=eps, mac_kind=B.MAC_ACCELERATION, mac_param=cfg["delta_acc"], aold=amag, amag_out=amag, r_crit=r_crit)
+    points = []
+    for frac in SWEEP_ACTIVE:
+        act = None if frac >= 1.0 else torch.from_numpy(W.random_active_subset(n, frac).astype(np.int32)).to(dev)
+        for ld in SWEEP_LOG2_DELTA:
+            kw = dict(eps=eps, mac_kind=B.MAC_ACCELERATION, mac_param=2.0 ** -ld, aold=amag, active=act, r_crit=r_crit)
+            cnt.zero_()
+            g.walk_tree(acc, n_interactions=cnt, **kw)          # warm-up + count
+            best = float("inf")
+            for _ in range(reps):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record()
+                g.walk_tree(acc, **kw)
+                b.record()
+                torch.cuda.synchronize()
+                best = min(best, a.elapsed_time(b))
+            ni = int(cnt.item())
+            points.append({"log2_delta_acc": -ld, "active_fraction": frac, "n_active": n if act is None else int(act.numel()), "walk_ms": best,
+                           "interactions": ni, "interactions_per_s": ni / (best * 1e-3),
+                           "frac_fp32_peak_24": ni / (best * 1e-3) * FLOP_PER_INTERACTION / 1e12 / alu_peak})
+    g.check()
+    g.close()
+    return {"n": n, "eps": eps, "r_crit": r_crit, "reps": reps, "timing": "best of reps, CUDA events around gothic_walk_tree (group marking included)", "points": points}
+
+
+def run_ours(args, rank: int, world: int, local_rank: int):
+    import torch
+    from paper_1610_07279_b200 import workloads as W
+    from paper_1610_07279_b200 import binding as B
+
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    peaks = _peaks()
+    props = torch.cuda.get_device_properties(dev)
+    m = measure_cycle(torch, W, B, args.workload, seed=args.seed + rank, n=args.n, r_crit=args.r_crit, steps=args.steps, warmup=args.warmup,
+                      dev=dev, barrier=barrier, clock_index=local_rank)
+    cfg, n, n_sub, n_levels, r_crit = m["cfg"], m["n"], m["n_sub"], m["n_levels"], m["r_crit"]
+    eps, dacc = cfg["eps"], cfg["delta_acc"]
+    total_ms, stage_ms, e2e, inter_total = m["total_ms"], m["stage_ms"], m["e2e"], m["inter_total"]
 
     # ---- max over ranks, aggregate ---------------------------------------------------------------------------------------
     (total_ms_max, walk_ms_max, e2e_ms_max), (inter_all, e2e_inter_all) = aggregate_over_ranks(
@@ -385,12 +490,17 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         walk_rate = inter_total / (stage_ms["walk"] * 1e-3)            # this rank's walk stage
         alu_peak = props.multi_processor_count * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12      # TFLOP/s, DESIGN.md "Rooflines"
         achieved = walk_rate * FLOP_PER_INTERACTION / 1e12
+        traffic, traffic_src = _walk_traffic(args.workload) if args.n is None else (None, None)
+        build_bytes = n * 309 + 0.24 * n * 150
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
             "ms_per_step": total_ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
-            "config": {"workload": args.workload, "n": n, "eps": eps, "delta_acc": dacc, "r_crit": r_crit, "eta": ETA, "max_levels": MAX_LEVELS, "seed": args.seed,
-                       "group_size": 32, "n_leaf": 16, "key": "peano_hilbert", "n_levels": n_levels, "n_substeps": n_sub,
+            "config": {"workload": args.workload, "n": n, "eps": eps, "delta_acc": dacc, "r_crit": r_crit,
+                       "r_crit_choice": "fixed per workload from a coarse sweep of the all-active walk time on a B200 (the paper auto-tunes it at run time, "
+                                        "PAPER.md:122-126); see DESIGN.md section 7",
+                       "eta": ETA, "max_levels": MAX_LEVELS, "seed": args.seed,
+                       "group_size": cfg["group_size"], "n_leaf": 16, "key": "peano_hilbert", "n_levels": n_levels, "n_substeps": n_sub,
                        "parallelism": "replicas" if world > 1 else "single_gpu", "l2": "inputs_exceed_l2" if n * 16 > 126e6 else "inputs_fit_l2"},
             "sec_per_block_step": total_ms_max * 1e-3 / K / n_sub,
             # the same with the tree build amortised three ways: rebuilt every block step, every 12 (the paper's
@@ -401,32 +511,43 @@ def run_ours(args, rank: int, world: int, local_rank: int):
                 "cycle": total_ms_max * 1e-3 / K / n_sub},
             "interactions_per_cycle": inter_total // K,
             "stage_ms_per_cycle": {k: v / K for k, v in stage_ms.items()},
-            "substeps": [{"substep": s + 1, "n_active": int(act_counts[s]), "interactions": int(inter_sub[s] // K),
-                          "walk_ms": walk_ms_sub[s] / K,
-                          "interactions_per_s": float(inter_sub[s] / max(walk_ms_sub[s], 1e-9) * 1e3)} for s in range(n_sub)],
+            "substeps": [{"substep": s + 1, "n_active": int(m["act_counts"][s]), "interactions": int(m["inter_sub"][s] // K),
+                          "walk_ms": m["walk_ms_sub"][s] / K,
+                          "interactions_per_s": float(m["inter_sub"][s] / max(m["walk_ms_sub"][s], 1e-9) * 1e3)} for s in range(n_sub)],
             "walk": {"interactions_per_s": walk_rate, "tflops_20": walk_rate * 20 / 1e12, "tflops_24": walk_rate * 24 / 1e12,
                      "tflops_28": walk_rate * 28 / 1e12, "frac_fp32_peak_24": achieved / alu_peak},
             "roofline": {"kernel": "k_walk", "bound": "alu", "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s", "frac": achieved / alu_peak,
-                         "traffic": NCU_WALK_TRAFFIC_BYTES.get(args.workload) if args.n is None else None, "traffic_unit": "bytes/launch",
+                         "traffic": traffic, "traffic_unit": "bytes/launch", "traffic_source": traffic_src,
                          "flop_per_interaction": FLOP_PER_INTERACTION,
-                         "avg_launch_ms": stage_ms["walk"] / max(walk_launches, 1),
+                         "avg_launch_ms": stage_ms["walk"] / max(m["walk_launches"], 1),
                          "peak_source": f"derived: {props.multi_processor_count} SM x 128 FP32 lanes x 2 flop x {peaks['sm_max_mhz']:.0f} MHz "
                                         f"(clock from MEASURED_PEAKS.json, {peaks['source']})"},
-            # the HBM-bound part: algorithmic bytes of one build (bbox 16, keys 16 + 8, histogram 8, 8 sort passes x 2 x 12,
+            # the HBM-bound part: algorithmic bytes of one build (bbox 16, keys 16 + 8, histogram 8, sort passes x 2 x 12,
             # gather 4 + 16 + 16, node events 2 x 8 B per particle; moments 16 + 16 + 4 + 1 B per particle and ~150 B per node)
-            "build_roofline": {"bound": "hbm", "achieved": (n * 309 + 0.24 * n * 150) / (stage_ms["build"] / K * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
-                               "unit": "GB/s", "frac": (n * 309 + 0.24 * n * 150) / (stage_ms["build"] / K * 1e-3) / 1e9 / peaks["hbm_gbs"],
+            "build_roofline": {"bound": "hbm", "achieved": build_bytes / (stage_ms["build"] / K * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
+                               "unit": "GB/s", "frac": build_bytes / (stage_ms["build"] / K * 1e-3) / 1e9 / peaks["hbm_gbs"],
                                "ms": stage_ms["build"] / K, "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peaks['source']})"},
-            "clocks": clk.summary(),
-            "gpu_launches": int(launches),
+            "clocks": m["clocks"],
+            "gpu_launches": m["launches"],
             "e2e": None,
         }
         if e2e:
             line["e2e"] = {"value": e2e_inter_all / (e2e_ms_max * 1e-3), "unit": UNIT, "h2d_bytes_per_step": e2e["h2d"],
                            "d2h_bytes_per_step": e2e["d2h"], "ms_per_step": e2e_ms_max / e2e["steps"], "steps": e2e["steps"]}
+        if world == 1 and not args.headline_only:
+            # the other BASELINE.json configs, a few steps each (north_star: "throughput on the synthetic models below")
+            others = {}
+            for name in OTHER_CONFIGS:
+                if name == args.workload:
+                    continue
+                mo = measure_cycle(torch, W, B, name, seed=args.seed, n=None, r_crit=None, steps=args.other_steps, warmup=3, dev=dev,
+                                   barrier=barrier, clock_index=local_rank, with_e2e=False)
+                others[name] = summarise(mo, alu_peak)
+                del mo
+            others["nfw_2p22_sweep"] = measure_sweep(torch, W, B, dev, alu_peak, args.seed)
+            line["other_configs"] = others
         if world == 1 and not args.no_cpu_baseline:
-            del g
-            line["cpu_baseline"] = cpu_baseline(pos_np, cfg, r_crit, args.cpu_budget)
+            line["cpu_baseline"] = cpu_baseline(m["pos_np"], cfg, r_crit, args.cpu_budget)
         print(json.dumps(line), flush=True)
     if dist is not None:
         dist.barrier()
@@ -444,6 +565,8 @@ def main():
     ap.add_argument("--seed", type=int, default=1)
     ap.add_argument("--r-crit", type=float, default=None, help="override the workload's critical separation (PAPER.md:122-126); inf = no group splitting")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--headline-only", action="store_true", help="skip the other BASELINE.json configs (other_configs)")
+    ap.add_argument("--other-steps", type=int, default=2, help="timed cycles of each of the other configs")
     ap.add_argument("--cpu-budget", type=float, default=15.0)
     ap.add_argument("--ref-groups", type=int, default=65536, help="i-groups per step of the --impl reference sample")
     args = ap.parse_args()

@@ -44,7 +44,7 @@ enum { GOTHIC_KEY_PEANO_HILBERT = 0, GOTHIC_KEY_MORTON = 1 };   /* PAPER.md:54 /
 enum { GOTHIC_BALL_GEO = 0, GOTHIC_BALL_EBS = 1, GOTHIC_BALL_COM = 2, GOTHIC_BALL_CMP = 3 };   /* enclosing ball of an i-group, App. B PAPER.md:568 items 3, 2, 4, 5 */
 enum { GOTHIC_MAC_ACCELERATION = 0, GOTHIC_MAC_OPENING_ANGLE = 1, GOTHIC_MAC_MULTIPOLE = 2 }; /* eq. 5 PAPER.md:85-89 / eq. 2 PAPER.md:68-72 / eq. 3-4 */
 
-/* Allocates a context for up to n_max particles.
+/* Allocates a context for up to n_max particles (n_max <= 2^30: the sort's look-back words carry 30-bit prefixes).
  *   node_max      node pool capacity; 0 -> 2*n_max (+64).  Must be < 2^28.
  *   group_size    G: number of consecutive sorted indices that share one traversal (PAPER.md:103-109,
  *                 "T_sub"; R3): 8, 16 or 32; 0 -> 32.  With G < 32 the spare lanes of the warp split
@@ -131,7 +131,8 @@ typedef struct {
 int gothic_get_tree_view(gothic_ctx *ctx, gothic_tree_view *out, void *stream);
 
 /* Synchronises `stream` and returns GOTHIC_ERR_CAPACITY / GOTHIC_ERR_CUDA if an asynchronous error was
- * flagged since the last check, else GOTHIC_OK. */
+ * flagged since the last check, else GOTHIC_OK.  The traversal-stack flag of a walk is sticky: it survives later
+ * builds and walks until a check reads (and clears) it, so one check after a whole cycle validates every walk in it. */
 int gothic_check(gothic_ctx *ctx, void *stream);
 
 /* End-to-end convenience with HOST buffers (bench.py "e2e"): H2D copy of pos_m (and aold), build, one walk of

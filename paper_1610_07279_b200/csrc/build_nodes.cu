@@ -249,7 +249,8 @@ int gothic_stage_nodes(gothic_ctx *c, uint32_t n, int n_leaf, cudaStream_t s)
 {
     const uint32_t nblk = (n + TPB - 1) / TPB;
     const uint64_t *key = c->key[c->cur];
-    GOTHIC_CUDA_OK(c, cudaMemsetAsync(c->flags, 0, 4 * sizeof(uint32_t), s));
+    // only the build's own overflow flag: flags[1] (the walk's stack overflow) stays set until gothic_check reads it, flags[2] is rewritten below
+    GOTHIC_CUDA_OK(c, cudaMemsetAsync(c->flags, 0, sizeof(uint32_t), s));
     k_count_events<<<nblk, TPB, 0, s>>>(key, n, n_leaf, c->blk_cnt, nblk);
     GOTHIC_LAUNCH_OK(c);
     k_scan_blocks<<<2 * GOTHIC_NLEVP1, SCAN_TPB, 0, s>>>(c->blk_cnt, nblk, c->level_cnt);

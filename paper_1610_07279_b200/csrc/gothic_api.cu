@@ -78,7 +78,7 @@ const char *gothic_last_cuda_error(gothic_ctx *ctx)
 
 int gothic_create(gothic_ctx **out, uint32_t n_max, uint32_t node_max, int group_size, size_t scratch_bytes)
 {
-    if (!out || n_max == 0 || n_max > (1u << 31)) return GOTHIC_ERR_ARG;
+    if (!out || n_max == 0 || n_max > (1u << 30)) return GOTHIC_ERR_ARG;   // the sort's look-back words carry 30-bit prefixes
     if (group_size == 0) group_size = 32;
     if (group_size != 8 && group_size != 16 && group_size != 32) return GOTHIC_ERR_ARG;
     if (node_max == 0) {
@@ -97,8 +97,7 @@ int gothic_create(gothic_ctx **out, uint32_t n_max, uint32_t node_max, int group
     cudaError_t e = cudaGetDevice(&c->device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device);
     if (e != cudaSuccess) { c->last_err = e; delete c; *out = nullptr; return GOTHIC_ERR_CUDA; }
-    gothic_walk_config(c);
-    gothic_sort_config();
+    if ((e = gothic_walk_config(c)) != cudaSuccess || (e = gothic_sort_config()) != cudaSuccess) { c->last_err = e; delete c; *out = nullptr; return GOTHIC_ERR_CUDA; }
     if (gothic_keys_config(c) != GOTHIC_OK) { delete c; *out = nullptr; return GOTHIC_ERR_CUDA; }
     c->stack_cap = 8192;   // u32 words of global spill area per resident warp (4096 families)
     if (scratch_bytes) {
@@ -330,7 +329,7 @@ int gothic_block_cycle_host(gothic_ctx *c, const float *pos_m_host, const float 
     GOTHIC_CUDA_OK(c, cudaMemcpyAsync(c->h2d_acc, acc_prev_host, b4, cudaMemcpyHostToDevice, c->copy_stream));
     GOTHIC_CUDA_OK(c, cudaEventRecord(c->copy_done, c->copy_stream));
     int rc = gothic_build_tree(c, reinterpret_cast<const float *>(c->h2d_pos), n, key_kind, n_leaf, stream);
-    if (rc != GOTHIC_OK) return rc;
+    if (rc != GOTHIC_OK) { cudaStreamSynchronize(c->copy_stream); return rc; }      // the caller's buffer is still being read
     GOTHIC_CUDA_OK(c, cudaStreamWaitEvent(s, c->copy_done, 0));
     const uint32_t grid = (n + 255u) / 256u;
     float *amag = c->d_aold_sorted;

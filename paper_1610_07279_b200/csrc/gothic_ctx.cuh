@@ -100,7 +100,7 @@ int gothic_stage_keys(gothic_ctx *c, const float4 *pos_m, uint32_t n, int key_ki
 int gothic_stage_sort(gothic_ctx *c, uint32_t n, cudaStream_t s);
 size_t gothic_sort_scratch_bytes(uint32_t n_max);
 int gothic_keys_config(gothic_ctx *c);     // uploads the Peano-Hilbert state table (called by gothic_create)
-void gothic_sort_config();                // per-device function attributes of the sort kernels (called by gothic_create)
+cudaError_t gothic_sort_config();         // per-device function attributes of the sort kernels (called by gothic_create)
 int gothic_stage_gather(gothic_ctx *c, const float4 *pos_m, uint32_t n, cudaStream_t s);
 int gothic_stage_nodes(gothic_ctx *c, uint32_t n, int n_leaf, cudaStream_t s);
 int gothic_stage_moments(gothic_ctx *c, cudaStream_t s);
@@ -112,7 +112,7 @@ int gothic_stage_walk(gothic_ctx *c, const uint32_t *active, uint32_t n_active, 
 int gothic_stage_timesteps(gothic_ctx *c, const float4 *acc_pot, uint32_t n, float cconst, int max_levels,
                            uint32_t substep, uint8_t *level, uint32_t *active, uint32_t *n_active_dev,
                            int32_t *emin_nlev_dev, cudaStream_t s);
-void gothic_walk_config(gothic_ctx *c);   // fills walk_warps / stack sizing (needs device properties)
+cudaError_t gothic_walk_config(gothic_ctx *c);   // function attributes + walk_warps (needs device properties)
 
 // ---- small device helpers -----------------------------------------------------------------------------
 __device__ __forceinline__ int shared_digits(uint64_t a, uint64_t b)

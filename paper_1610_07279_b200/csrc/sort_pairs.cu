@@ -205,10 +205,11 @@ size_t gothic_sort_scratch_bytes(uint32_t n_max)
     return (sort_words_head() + (size_t)NPASS * ntiles * RADIX) * sizeof(uint32_t);
 }
 
-void gothic_sort_config()
+cudaError_t gothic_sort_config()
 {
-    cudaFuncSetAttribute(k_sort_onesweep, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem));
-    cudaFuncSetAttribute(k_sort_onesweep, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    cudaError_t e = cudaFuncSetAttribute(k_sort_onesweep, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SortSmem));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_sort_onesweep, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    return e;
 }
 
 int gothic_stage_sort(gothic_ctx *c, uint32_t n, cudaStream_t s)

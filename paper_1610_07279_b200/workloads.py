@@ -158,12 +158,14 @@ def random_active_subset(n: int, fraction: float, seed: int = 7) -> np.ndarray:
 # name -> (generator, N, eps, delta_acc, description) : BASELINE.json "configs" in order
 CONFIGS = {
     # r_crit: critical separation for splitting wide i-groups.  The paper tunes it at run time from
-    # timings; here it is a fixed number per workload, found once by a sweep on a B200.
-    "plummer_2p13": dict(model=plummer, n=1 << 13, eps=1.0 / 64, delta_acc=2.0 ** -7, block=False, r_crit=1.0),
-    "hernquist_2p20": dict(model=hernquist, n=1 << 20, eps=2.0 ** -7, delta_acc=2.0 ** -9, block=False, r_crit=0.5),
-    "nfw_2p24_block": dict(model=nfw, n=1 << 24, eps=2.0 ** -8, delta_acc=2.0 ** -9, block=True, r_crit=0.5),
-    "m31_2p24_block": dict(model=m31_like, n=1 << 24, eps=2.0 ** -8, delta_acc=2.0 ** -9, block=True, r_crit=0.5),
-    "nfw_2p22_sweep": dict(model=nfw, n=1 << 22, eps=2.0 ** -8, delta_acc=2.0 ** -9, block=False, r_crit=0.5),
+    # timings (Brent's method); here it is a fixed number per workload, picked from a coarse sweep of the all-active walk time on
+    # a B200 ("r_crit": NFW 0.125 ... 2, Hernquist 0.25 ... 64).  group_size: G of reading R3; a problem too
+    # small to give every resident warp a group takes G = 8 (S = 4 lanes per i-particle).
+    "plummer_2p13": dict(model=plummer, n=1 << 13, eps=1.0 / 64, delta_acc=2.0 ** -7, block=False, r_crit=1.0, group_size=8),
+    "hernquist_2p20": dict(model=hernquist, n=1 << 20, eps=2.0 ** -7, delta_acc=2.0 ** -9, block=False, r_crit=16.0, group_size=32),
+    "nfw_2p24_block": dict(model=nfw, n=1 << 24, eps=2.0 ** -8, delta_acc=2.0 ** -9, block=True, r_crit=0.5, group_size=32),
+    "m31_2p24_block": dict(model=m31_like, n=1 << 24, eps=2.0 ** -8, delta_acc=2.0 ** -9, block=True, r_crit=0.5, group_size=32),
+    "nfw_2p22_sweep": dict(model=nfw, n=1 << 22, eps=2.0 ** -8, delta_acc=2.0 ** -9, block=False, r_crit=0.5, group_size=32),
 }
 
 

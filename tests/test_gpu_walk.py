@@ -337,3 +337,23 @@ def test_walk_randomised_parity_sweep(oracle):
         assert cnt == c["interactions"], (it, model, n, G, n_leaf, frac, r_crit, ball, kind, param)
         _assert_parity(out, ref, rows)
         g.close()
+
+
+def test_stack_overflow_flag_survives_a_rebuild(oracle):
+    """gothic.h: the traversal-stack overflow flag is sticky until gothic_check reads it (a rebuild must not lose it)."""
+    import torch
+    from gpu_util import dev
+    from paper_1610_07279_b200.binding import Gothic, GothicError
+    n = 1 << 17
+    pos = W.plummer(n, seed=4)
+    g = Gothic(n, scratch_bytes=512 * 4 * 148 * 64)      # the smallest spill areas gothic_create accepts (>= 512 words per warp)
+    d_pos = dev(pos)
+    g.build_tree(d_pos, n_leaf=1)
+    acc = torch.zeros(n, 4, device="cuda")
+    # theta = 0 opens every node: with one particle per leaf the pending families outgrow the 256 + 256 slots of a warp
+    g.walk_tree(acc, eps=0.01, mac_kind=1, mac_param=0.0, active=torch.arange(0, 64, dtype=torch.int32, device="cuda"))
+    g.build_tree(d_pos, n_leaf=1)        # a rebuild between the walk and the check
+    with pytest.raises(GothicError, match="capacity"):
+        g.check()
+    g.check()                            # read and cleared
+    g.close()
