@@ -30,6 +30,40 @@ def _group_samples(n, per=64, pieces=4):
     return [(lo, lo + per) for lo in np.linspace(0, n_groups - per, pieces).astype(int)]
 
 
+def _seeded_group_ids(pos_sorted, seed, places=16, run=8, widest=8):
+    """Group ids for the count-equality checks: `places` seeded random runs of `run` consecutive groups plus the `widest` groups
+    with the largest GEO ball (the ones r_crit splits the deepest)."""
+    n = pos_sorted.shape[0]
+    n_groups = n // G
+    rng = np.random.default_rng(seed)
+    starts = rng.choice(n_groups - run, places, replace=False)
+    ids = np.concatenate([np.arange(s0, s0 + run) for s0 in starts])
+    xyz = pos_sorted[: n_groups * G, :3].reshape(n_groups, G, 3)
+    ctr = 0.5 * (xyz.min(axis=1) + xyz.max(axis=1))
+    r2 = ((xyz - ctr[:, None, :]) ** 2).sum(axis=2).max(axis=1)
+    ids = np.concatenate([ids, np.argsort(r2)[-widest:]])
+    return np.unique(ids).astype(np.int64)
+
+
+def _count_equality(g, oracle_walk, gids, members, n, *, eps, dacc, aold, r_crit, out_full, active=None):
+    """Walks ONLY `members` (the active particles of the groups `gids`) on the GPU with its own device counter and holds the count
+    against the oracle's sum over the same groups: EQUAL, the sharpest check of the suite, here at full size.  The rows of that
+    restricted walk are also bit-identical to the full walk's (a group's arithmetic does not depend on which other groups walk)."""
+    from gpu_util import dev
+    from paper_1610_07279_b200.binding import MAC_ACCELERATION
+    acc2 = torch.zeros(n, 4, device="cuda")
+    cnt2 = torch.zeros(1, dtype=torch.int64, device="cuda")
+    g.walk_tree(acc2, eps=eps, mac_kind=MAC_ACCELERATION, mac_param=dacc, aold=dev(aold), active=dev(members.astype(np.uint32), torch.int32),
+                r_crit=r_crit, n_interactions=cnt2)
+    g.check()
+    total = 0
+    for gid in gids:
+        _, c = oracle_walk(eps=eps, mac_kind=0, mac_param=dacc, aold=aold, active=active, group_range=(int(gid), int(gid) + 1), r_crit=r_crit)
+        total += c["interactions"]
+    assert int(cnt2.item()) == total, (int(cnt2.item()), total)
+    assert np.array_equal(acc2.cpu().numpy()[members], out_full[members].astype(np.float32))
+
+
 def _rows_of(ranges, active=None):
     rows = np.concatenate([np.arange(lo * G, hi * G) for lo, hi in ranges])
     if active is not None:
@@ -81,6 +115,9 @@ def test_block_cycle_full_size(oracle, name):
     mom = np.linalg.norm((m[:, None] * out[:, :3]).sum(0)) / (m * np.linalg.norm(out[:, :3], axis=1)).sum()
     assert mom < 2e-3, mom                       # momentum near-conservation (north_star)
     assert 800 < int(cnt.item()) / n < 4000      # interactions per particle at Delta_acc = 2^-9
+    gids = _seeded_group_ids(v["pos_m_sorted"], seed=20261105)
+    members = np.concatenate([np.arange(gid * G, (gid + 1) * G) for gid in gids])
+    _count_equality(g, oracle_walk, gids, members, n, eps=eps, dacc=dacc, aold=aold, r_crit=r_crit, out_full=out)
     # ---- T1: levels bit-exact over all N ----
     level = torch.zeros(n, dtype=torch.uint8, device="cuda")
     active = torch.zeros(n, dtype=torch.int32, device="cuda")
@@ -109,6 +146,15 @@ def test_block_cycle_full_size(oracle, name):
             rows = _rows_of([(lo, hi)], act_ref)
             if rows.size:
                 _parity(out, ref, rows)
+        if s in (1, 2, 2 ** (nlev - 1)):          # count equality on seeded groups, incl. the sparsest member masks of this substep
+            per_group = np.bincount(act_ref // G, minlength=n // G)
+            lonely = np.flatnonzero(per_group == 1)
+            rng = np.random.default_rng(100 + s)
+            gs = np.unique(np.concatenate([gids, rng.choice(lonely, min(8, lonely.size), replace=False) if lonely.size else gids[:0]]))
+            gs = gs[per_group[gs] > 0]
+            members = act_ref[np.isin(act_ref // G, gs)]
+            if members.size:
+                _count_equality(g, oracle_walk, gs, members, n, eps=eps, dacc=dacc, aold=aold, r_crit=r_crit, out_full=out, active=act_ref)
         inactive = torch.ones(n, dtype=torch.bool, device="cuda")
         inactive[active[:na].long()] = False
         assert torch.equal(acc[inactive], before[inactive])     # only active rows are written

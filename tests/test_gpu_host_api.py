@@ -59,6 +59,46 @@ def test_block_cycle_host_equals_device_calls(oracle, model, n):
     g.close()
 
 
+@pytest.mark.parametrize("model,n", [("plummer", 20000), ("hernquist", 30011)])
+def test_block_cycle_host_vs_oracle(oracle, model, n):
+    """The e2e call itself against the oracle, nothing of the CUDA path on the reference side: the oracle builds its own tree and moments,
+    takes the levels from the same previous accelerations and walks every substep's active set with its own running |a_old|.  Levels and
+    the substep count are bit-exact; accelerations within the north_star tolerances (MAC flips at threshold allowed), counts to 1e-3."""
+    from paper_1610_07279_b200.binding import Gothic
+    pos = getattr(W, model)(n, seed=6)
+    eps, dacc, eta, max_levels, r_crit = 2.0 ** -6, 2.0 ** -8, 0.5, 6, 0.5
+    t = oracle.build_tree(pos)
+    boot, _ = oracle.walk_tree(t, eps=eps, mac_kind=1, mac_param=0.5)
+    acc_prev = np.zeros((n, 4), np.float32)
+    acc_prev[t.perm] = boot.astype(np.float32)                 # ORIGINAL order
+    # ---- the cycle in the oracle (sorted order) ----
+    acc_s = acc_prev[t.perm]
+    lev_s, e_min, nlev = oracle.levels(acc_s, eps, eta, max_levels)
+    amag = np.sqrt(np.float32(np.float64(acc_s[:, 2]) ** 2 + np.float32(np.float64(acc_s[:, 1]) ** 2 + np.float32(acc_s[:, 0] * acc_s[:, 0]))).astype(np.float32))
+    ref = acc_s.astype(np.float64)
+    total = 0
+    for s in range(1, 2 ** (nlev - 1) + 1):
+        act = oracle.active_set(lev_s, s)
+        o, c = oracle.walk_tree(t, eps=eps, mac_kind=0, mac_param=dacc, aold=amag, active=act, r_crit=r_crit)
+        ref[act] = o[act]
+        amag[act] = np.linalg.norm(o[act, :3], axis=1).astype(np.float32)
+        total += c["interactions"]
+    # ---- the host call ----
+    g = Gothic(n)
+    h_out, h_lev = torch.empty(n, 4).pin_memory(), torch.empty(n, dtype=torch.uint8).pin_memory()
+    info = g.block_cycle_host(torch.from_numpy(pos).pin_memory(), torch.from_numpy(acc_prev).pin_memory(), h_out, eps=eps, delta_acc=dacc, eta=eta,
+                              max_levels=max_levels, level_host=h_lev, count=True, r_crit=r_crit)
+    g.check()
+    assert (info["e_min"], info["n_levels"], info["n_substeps"]) == (e_min, nlev, 2 ** (nlev - 1))
+    assert np.array_equal(h_lev.numpy()[t.perm], lev_s)
+    out = h_out.numpy().astype(np.float64)[t.perm]
+    e = np.linalg.norm(out[:, :3] - ref[:, :3], axis=1) / np.linalg.norm(ref[:, :3], axis=1)
+    pe = np.abs(out[:, 3] - ref[:, 3]) / np.abs(ref[:, 3])
+    assert np.percentile(e, 99.9) <= 1e-4 and e.max() <= 1e-2 and np.median(pe) <= 1e-4, (np.percentile(e, 99.9), e.max(), np.median(pe))
+    assert abs(info["interactions"] - total) <= 1e-3 * total, (info["interactions"], total)
+    g.close()
+
+
 def test_gravity_host_equals_device_calls():
     from paper_1610_07279_b200.binding import Gothic, MAC_ACCELERATION, MAC_OPENING_ANGLE
     n = 30000

@@ -174,6 +174,25 @@ def test_walk_end_to_end_tolerances_and_error_vs_direct(oracle):
     g.close()
 
 
+def test_walk_end_to_end_hernquist_full_size(oracle):
+    """BASELINE.json configs[1] (Hernquist 2^20, eps 2^-7, Delta_acc 2^-9) END TO END at full size: the oracle builds its OWN tree and
+    its OWN moments (double sums) and walks all 2^20 particles; the CUDA path is held to the north_star tolerances with MAC flips at
+    threshold allowed, and the interaction counts agree to 1e-3."""
+    from gpu_util import gpu_build, gpu_walk
+    pos, cfg = W.make_config("hernquist_2p20", seed=1)
+    n, eps, dacc, r_crit = cfg["n"], cfg["eps"], cfg["delta_acc"], cfg["r_crit"]
+    g, v = gpu_build(pos)
+    t = oracle.build_tree(pos)
+    assert np.array_equal(v["perm"], t.perm)
+    boot, _ = oracle.walk_tree(t, eps=eps, mac_kind=1, mac_param=0.5, r_crit=r_crit)
+    aold = np.linalg.norm(boot[:, :3], axis=1).astype(np.float32)
+    ref, c = oracle.walk_tree(t, eps=eps, mac_kind=0, mac_param=dacc, aold=aold, r_crit=r_crit)
+    out, cnt, _ = gpu_walk(g, n, eps=eps, mac_kind=0, mac_param=dacc, aold=aold, r_crit=r_crit)
+    _assert_parity(out, ref, np.arange(n))
+    assert abs(cnt - c["interactions"]) <= 1e-3 * c["interactions"], (cnt, c["interactions"])
+    g.close()
+
+
 def test_walk_full_size_hernquist_sampled(oracle):
     """BASELINE.json configs[1] at full size (N = 2^20) in the bench launch configuration; the oracle walks a
     sample of groups on the GPU-built tree, all sampled particles compared one by one."""
@@ -267,7 +286,11 @@ def test_walk_ebs_ball_matches_oracle(oracle, model, n, G, frac, r_crit):
         _assert_parity(out, ref, rows)
     g.set_ball(BALL_GEO)
     _, cnt_geo, _ = gpu_walk(g, n, eps=eps, mac_kind=0, mac_param=2.0 ** -8, aold=aold, active=active, r_crit=r_crit)
-    assert counts[0] != cnt_geo and abs(counts[0] - cnt_geo) < 0.2 * cnt_geo       # a different, slightly tighter ball
+    # Not a parity tolerance (the counts above are EQUAL to the oracle's): a sanity bound that EBS really is another ball of about the
+    # same size.  Fig. B.10 of the paper puts the interaction counts of the enclosing balls within ~10 % of each other at
+    # full groups; the sparse cases here (6 % active at G = 8) have one- and two-member pieces whose balls, and with them the counts,
+    # differ by up to 14 % between Ritter's sphere and the bounding-cuboid centre, hence 20 %.
+    assert counts[0] != cnt_geo and abs(counts[0] - cnt_geo) < 0.2 * cnt_geo
     g.close()
 
 
