@@ -2,6 +2,7 @@
 """bench.py -- whole-hot-path benchmark of the B200-native GOTHIC block-step cycle (driver contract).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME] [--n N]
+    python bench.py --workload nfw_2p22_live | plummer_2p20_live | nfw_2p24_live      (live block stepping only, see measure_live)
 
 A "step" is one full block-step CYCLE of the workload (BASELINE.json configs[2], NFW sphere N = 2^24 by default):
     gothic_build_tree                                  (B1-B6: bbox, keys, sort, gather, nodes, moments)
@@ -454,6 +455,59 @@ def measure_sweep(torch, W, B, dev, alu_peak: float, seed: int, reps: int = 3) -
     return {"n": n, "eps": eps, "r_crit": r_crit, "reps": reps, "timing": "best of reps, CUDA events around gothic_walk_tree (group marking included)", "points": points}
 
 
+def measure_live(torch, W, B, workload: str, *, seed: int, n, dev, alu_peak: float, intervals=(1, 2, 4, 12, "cycle"), cycles: int = 2) -> dict:
+    """The paper's actual time-to-solution loop with MOVING particles through gothic_live_step: per block
+    step predict all -> rebuild (every k-th step) or moments refresh -> active list -> walk -> correct with level migration, state on the
+    device in tree order.  For each rebuild interval k: one warm-up cycle, then `cycles` block cycles timed with CUDA events
+    (seconds per block step), then one more cycle replayed with the interaction counter read after every step (separate run)."""
+    pos_np, vel_np, cfg = W.make_live_config(workload, seed=seed, n=n)
+    n, eps, dacc, r_crit = cfg["n"], cfg["eps"], cfg["delta_acc"], cfg["r_crit"]
+    pos, vel = torch.from_numpy(pos_np).to(dev), torch.from_numpy(vel_np).to(dev)
+    out = {"workload": workload, "n": n, "eps": eps, "delta_acc": dacc, "r_crit": r_crit, "eta": ETA, "max_levels": MAX_LEVELS, "cycles_timed": cycles,
+           "velocities": "isotropic Gaussian, Jeans dispersion of the truncated profile (workloads.isotropic_velocities)", "rebuild_every": {}}
+    for k in intervals:
+        g = B.Gothic(n, group_size=cfg["group_size"])
+        g.live_init(pos, vel, eps=eps, eta=ETA, max_levels=MAX_LEVELS, theta_boot=THETA_BOOTSTRAP)
+
+        def run_cycle(counter=None, log=None):
+            st = g.live_get(arrays=False)
+            for s in range(st["n_substeps"]):
+                rebuild = (s == 0) if k == "cycle" else (st["steps"] + s) % k == 0
+                g.live_step(delta_acc=dacc, r_crit=r_crit, rebuild=rebuild, n_interactions=counter)
+                if log is not None:
+                    now = g.live_get(arrays="n_active")
+                    log.append((s + 1, int(now["steps_since_rebuild"]), int(now["n_active"].item()), int(counter.item())))
+            return st["n_substeps"]
+
+        run_cycle()                       # warm-up
+        g.check()
+        launches0 = g.launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        steps = 0
+        for _ in range(cycles):
+            steps += run_cycle()
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+        launches = g.launch_count() - launches0
+        g.check()
+        counter = torch.zeros(1, dtype=torch.int64, device=dev)
+        log = []
+        n_sub = run_cycle(counter, log)
+        g.check()
+        inter = [b[3] - a for a, b in zip([0] + [x[3] for x in log[:-1]], log)]
+        total = int(counter.item())
+        out["rebuild_every"][str(k)] = {
+            "sec_per_block_step": ms * 1e-3 / steps, "ms_per_cycle": ms / cycles, "block_steps_timed": steps, "n_substeps_last_cycle": n_sub,
+            "interactions_per_cycle": total, "interactions_per_s": total * cycles / (ms * 1e-3) if steps == n_sub * cycles else None,
+            "gpu_launches_per_step": launches / steps,
+            "steps": [{"substep": a, "steps_since_rebuild": b, "n_active": c, "interactions": i} for (a, b, c, _), i in zip(log, inter)]}
+        g.close()
+    return out
+
+
 def run_ours(args, rank: int, world: int, local_rank: int):
     import torch
     from paper_1610_07279_b200 import workloads as W
@@ -474,6 +528,23 @@ def run_ours(args, rank: int, world: int, local_rank: int):
 
     peaks = _peaks()
     props = torch.cuda.get_device_properties(dev)
+    if args.workload.endswith("_live"):
+        # live block stepping only: one line whose headline is the run with the tree rebuilt once per block cycle
+        alu_peak = props.multi_processor_count * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+        with ClockSampler(local_rank) as clk:
+            lv = measure_live(torch, W, B, args.workload, seed=args.seed + rank, n=args.n, dev=dev, alu_peak=alu_peak, cycles=max(1, args.steps))
+        head = lv["rebuild_every"]["cycle"]
+        (ms_max,), (inter_all,) = aggregate_over_ranks(dist, [head["ms_per_cycle"]], [head["interactions_per_cycle"]], dev)
+        if rank == 0:
+            print(json.dumps({"metric": METRIC, "value": inter_all / (ms_max * 1e-3), "unit": UNIT, "n_gpus": world, "steps": max(1, args.steps),
+                              "warmup": 1, "ms_per_step": ms_max, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+                              "data": "synthetic", "config": {"workload": args.workload, "n": lv["n"], "parallelism": "replicas" if world > 1 else "single_gpu"},
+                              "sec_per_block_step": head["sec_per_block_step"], "live": lv, "clocks": clk.summary(),
+                              "gpu_launches": int(head["gpu_launches_per_step"] * head["block_steps_timed"])}), flush=True)
+        if dist is not None:
+            dist.barrier()
+            dist.destroy_process_group()
+        return
     m = measure_cycle(torch, W, B, args.workload, seed=args.seed + rank, n=args.n, r_crit=args.r_crit, steps=args.steps, warmup=args.warmup,
                       dev=dev, barrier=barrier, clock_index=local_rank)
     cfg, n, n_sub, n_levels, r_crit = m["cfg"], m["n"], m["n_sub"], m["n_levels"], m["r_crit"]
@@ -546,6 +617,8 @@ def run_ours(args, rank: int, world: int, local_rank: int):
                 del mo
             others["nfw_2p22_sweep"] = measure_sweep(torch, W, B, dev, alu_peak, args.seed)
             line["other_configs"] = others
+            # the same sphere with moving particles: predict -> rebuild / refresh -> walk -> correct (gothic_live_step), SURVEY.md 8f row 1
+            line["live"] = measure_live(torch, W, B, "nfw_2p24_live", seed=args.seed, n=None, dev=dev, alu_peak=alu_peak, intervals=(1, 2, 4, "cycle"), cycles=2)
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(m["pos_np"], cfg, r_crit, args.cpu_budget)
         print(json.dumps(line), flush=True)

@@ -190,6 +190,45 @@ int gothic_correct(gothic_ctx *ctx, const uint32_t *active, uint32_t n_active, c
                    float *acc_pot, uint32_t *t_last, uint8_t *level, float eps, float eta, int e_min, int max_levels,
                    void *stream);
 
+/* Live block time stepping: the paper's per-step loop with MOVING particles, state kept on the
+ * device by the library in tree order.  One gothic_live_step is one block step: t_now += 1 (in units of dt_unit = 2^e_min),
+ *   predict ALL particles to t_now (eq. 15-16) -> tree: rebuild from the predicted positions (and re-order the state by the new
+ *   permutation), or keep the links and only recompute the pseudo-j moments from the predicted positions ->
+ *   active list of the substep (level <= ctz(t_now)) -> walk of the active particles with the acceleration MAC (eq. 5,
+ *   |a_old| = the particle's last |a|) -> correct the active particles (eq. 17) with level migration (reading R15).
+ * When t_now reaches n_substeps = 2^(n_levels-1) every particle is synchronised: the levels are taken afresh from the new
+ * accelerations (gothic_set_timesteps' arithmetic), t_now and every t_last return to 0, and one 8-byte read-back of
+ * {e_min, n_levels} synchronises the stream (once per cycle).  Everything else is asynchronous.
+ *
+ * gothic_live_init: pos_m float4[n], vel float4[n] (vx, vy, vz, unused) in ORIGINAL order; builds the tree, bootstraps the
+ *   accelerations with an opening-angle walk (eq. 2, theta_boot; R7), takes the first levels.  Synchronises.
+ * gothic_live_step: rebuild != 0 rebuilds the tree in this step.  n_interactions (device, optional) accumulates P:331's count.
+ * gothic_live_get: device pointers of the current state (tree order; orig[s] = original index of row s) and the clock.
+ *   The pointers stay valid until the next rebuild step or gothic_live_init; rows change with every step.
+ * Errors: GOTHIC_ERR_STATE before gothic_live_init; GOTHIC_ERR_ARG for bad arguments. */
+typedef struct gothic_live_state {
+    uint32_t n;
+    uint32_t t_now;               /* substep index within the cycle, 0 .. n_substeps */
+    uint32_t n_substeps;          /* 2^(n_levels-1) */
+    int32_t e_min;                /* dt_unit = 2^e_min */
+    int32_t n_levels;
+    uint32_t steps_since_rebuild;
+    unsigned long long steps;     /* block steps taken since gothic_live_init */
+    const float *pos_m;           /* float4[n]: position at the row's own t_last, mass */
+    const float *vel;             /* float4[n] */
+    const float *acc_pot;         /* float4[n]: (ax, ay, az, Phi) at t_last */
+    const float *amag;            /* float[n]: |a|, the next walk's |a_old| */
+    const uint32_t *t_last;       /* uint32[n] */
+    const uint8_t *level;         /* uint8[n] */
+    const uint32_t *orig;         /* uint32[n] */
+    const uint32_t *active;       /* uint32[n_active]: active rows of the last step (ascending) */
+    const uint32_t *n_active;     /* device count of `active` */
+} gothic_live_state;
+int gothic_live_init(gothic_ctx *ctx, const float *pos_m, const float *vel, uint32_t n, int key_kind, int n_leaf, float eps,
+                     float eta, int max_levels, float theta_boot, void *stream);
+int gothic_live_step(gothic_ctx *ctx, float delta_acc, float r_crit, int rebuild, unsigned long long *n_interactions, void *stream);
+int gothic_live_get(gothic_ctx *ctx, gothic_live_state *out);
+
 /* Number of kernels this library has launched through this context (bench.py "gpu_launches"). */
 unsigned long long gothic_launch_count(gothic_ctx *ctx);
 

@@ -21,6 +21,7 @@ EXPORTS = [
     "gothic_create", "gothic_destroy", "gothic_strerror", "gothic_last_cuda_error", "gothic_build_tree",
     "gothic_update_moments", "gothic_walk_tree", "gothic_set_timesteps", "gothic_get_tree_view", "gothic_check",
     "gothic_gravity_host", "gothic_block_cycle_host", "gothic_launch_count", "gothic_predict", "gothic_correct", "gothic_set_ball",
+    "gothic_live_init", "gothic_live_step", "gothic_live_get",
 ]
 
 
@@ -35,6 +36,13 @@ class TreeViewStruct(C.Structure):
                 ("node_head", C.c_void_p), ("node_num", C.c_void_p), ("node_child", C.c_void_p),
                 ("node_level", C.c_void_p), ("node_nchild", C.c_void_p), ("level_ofs", C.c_void_p),
                 ("node_com", C.c_void_p), ("node_b", C.c_void_p), ("node_b2", C.c_void_p)]
+
+
+class LiveStateStruct(C.Structure):
+    _fields_ = [("n", C.c_uint32), ("t_now", C.c_uint32), ("n_substeps", C.c_uint32), ("e_min", C.c_int32), ("n_levels", C.c_int32),
+                ("steps_since_rebuild", C.c_uint32), ("steps", C.c_ulonglong),
+                ("pos_m", C.c_void_p), ("vel", C.c_void_p), ("acc_pot", C.c_void_p), ("amag", C.c_void_p), ("t_last", C.c_void_p),
+                ("level", C.c_void_p), ("orig", C.c_void_p), ("active", C.c_void_p), ("n_active", C.c_void_p)]
 
 
 _lib = None
@@ -79,6 +87,12 @@ def load_library():
     L.gothic_predict.argtypes = [vp, vp, vp, vp, vp, u32, f32, u32, vp, vp]
     L.gothic_correct.restype = i32
     L.gothic_correct.argtypes = [vp, vp, u32, vp, u32, vp, vp, u32, f32, vp, vp, vp, vp, vp, f32, f32, i32, i32, vp]
+    L.gothic_live_init.restype = i32
+    L.gothic_live_init.argtypes = [vp, vp, vp, u32, i32, i32, f32, f32, i32, f32, vp]
+    L.gothic_live_step.restype = i32
+    L.gothic_live_step.argtypes = [vp, f32, f32, i32, vp, vp]
+    L.gothic_live_get.restype = i32
+    L.gothic_live_get.argtypes = [vp, C.POINTER(LiveStateStruct)]
     L.gothic_launch_count.restype = C.c_ulonglong
     L.gothic_launch_count.argtypes = [vp]
     _lib = L
@@ -212,6 +226,32 @@ class Gothic:
             node_nchild=_from_ptr(v.node_nchild, m, torch.uint8, d), level_ofs=_from_ptr(v.level_ofs, 23, torch.int32, d),
             node_com=_from_ptr(v.node_com, 4 * m, torch.float32, d).view(m, 4), node_b=_from_ptr(v.node_b, m, torch.float32, d), node_b2=_from_ptr(v.node_b2, m, torch.float32, d),
         )
+
+    def live_init(self, pos_m: torch.Tensor, vel: torch.Tensor, *, eps: float, eta: float = 0.5, max_levels: int = 8, theta_boot: float = 0.5,
+                  key_kind: int = KEY_PEANO_HILBERT, n_leaf: int = 16):
+        """Live block stepping (gothic_live_*): state kept on the device by the library, in tree order."""
+        self._chk(self._L.gothic_live_init(self._ctx, _ptr(pos_m, torch.float32), _ptr(vel, torch.float32), pos_m.shape[0], key_kind, n_leaf,
+                                           float(eps), float(eta), int(max_levels), float(theta_boot), _stream()))
+
+    def live_step(self, *, delta_acc: float, r_crit: float = float("inf"), rebuild: bool = False, n_interactions: torch.Tensor | None = None):
+        self._chk(self._L.gothic_live_step(self._ctx, float(delta_acc), float(r_crit), int(bool(rebuild)), _ptr(n_interactions, torch.int64), _stream()))
+
+    def live_get(self, arrays: bool | str = True) -> dict:
+        """The clock of the live run and (arrays=True) copies of its state rows in tree order (tests, diagnostics); arrays="n_active": only the
+        device count of the last step's active list."""
+        v = LiveStateStruct()
+        self._chk(self._L.gothic_live_get(self._ctx, C.byref(v)))
+        d, n = self.device, v.n
+        out = dict(n=n, t_now=v.t_now, n_substeps=v.n_substeps, e_min=v.e_min, n_levels=v.n_levels, steps_since_rebuild=v.steps_since_rebuild, steps=v.steps)
+        if arrays == "n_active":
+            out.update(n_active=_from_ptr(v.n_active, 1, torch.int32, d))
+        elif arrays:
+            torch.cuda.current_stream().synchronize()
+            out.update(pos_m=_from_ptr(v.pos_m, 4 * n, torch.float32, d).view(n, 4), vel=_from_ptr(v.vel, 4 * n, torch.float32, d).view(n, 4),
+                       acc_pot=_from_ptr(v.acc_pot, 4 * n, torch.float32, d).view(n, 4), amag=_from_ptr(v.amag, n, torch.float32, d),
+                       t_last=_from_ptr(v.t_last, n, torch.int32, d), level=_from_ptr(v.level, n, torch.uint8, d), orig=_from_ptr(v.orig, n, torch.int32, d),
+                       active=_from_ptr(v.active, n, torch.int32, d), n_active=_from_ptr(v.n_active, 1, torch.int32, d))
+        return out
 
     def gravity_host(self, pos_m_host: torch.Tensor, acc_pot_host: torch.Tensor, *, eps: float, mac_kind: int, mac_param: float,
                      aold_host: torch.Tensor | None = None, perm_host: torch.Tensor | None = None,

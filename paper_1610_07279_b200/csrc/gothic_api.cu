@@ -20,6 +20,7 @@ void free_all(gothic_ctx *c)
                     c->level_ofs, c->level_cnt, c->blk_cnt, c->flags, c->sort_tmp, c->grp_mask, c->grp_list, c->grp_cnt,
                     c->stack, c->ts_tmp, c->scan_tmp, c->h2d_pos, c->h2d_aold, c->d_aold_sorted, c->d_acc,
                     c->h2d_acc, c->d_level, c->d_active, c->d_cycle_info, c->d_count};
+    gothic_live_free(c);
     for (void *p : ptrs)
         if (p) cudaFree(p);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);

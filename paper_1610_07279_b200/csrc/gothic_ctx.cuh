@@ -80,7 +80,9 @@ struct gothic_ctx {
     cudaStream_t copy_stream; cudaEvent_t copy_done;   // second copy queue of gothic_block_cycle_host (overlaps H2D with the build)
     // extra staging for gothic_block_cycle_host
     float4 *h2d_acc; uint8_t *d_level; uint32_t *d_active; int32_t *d_cycle_info; unsigned long long *d_count;
+    struct gothic_live *live;   // state of gothic_live_* (integrate.cu), NULL until gothic_live_init
 };
+void gothic_live_free(gothic_ctx *c);
 
 #define GOTHIC_CUDA_OK(ctx, expr)                                   \
     do {                                                            \

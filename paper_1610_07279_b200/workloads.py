@@ -14,7 +14,7 @@ from __future__ import annotations
 import numpy as np
 
 __all__ = [
-    "plummer", "hernquist", "nfw", "m31_like", "make_config", "CONFIGS", "random_active_subset",
+    "plummer", "hernquist", "nfw", "m31_like", "make_config", "CONFIGS", "random_active_subset", "isotropic_velocities", "LIVE_CONFIGS", "make_live_config",
 ]
 
 
@@ -144,6 +144,32 @@ def m31_like(n: int, seed: int = 1) -> np.ndarray:
     return _finish(rng, xyz)
 
 
+def isotropic_velocities(pos_m: np.ndarray, model: str, seed: int = 2) -> np.ndarray:
+    """Velocities (vx, vy, vz, 0) float32 for the live block-stepping runs: isotropic Gaussian with the local radial dispersion of the
+    spherical Jeans equation, sigma^2(r) = (1/rho) int_r^rmax rho(s) M(<s) / s^2 ds (G = 1, total mass 1 inside the cut), integrated
+    numerically on a logarithmic grid for the truncated profile.  A near-equilibrium start, not an exact distribution function:
+    enough for the orbits, level migration and tree ageing of a time-to-solution measurement.  model: plummer | hernquist | nfw."""
+    r = np.linalg.norm(pos_m[:, :3].astype(np.float64), axis=1)
+    if model == "plummer":
+        rmax, rho, mass = 20.0, (lambda x: (1.0 + x * x) ** -2.5), (lambda x: x ** 3 / (1.0 + x * x) ** 1.5)
+    elif model == "hernquist":
+        rmax, rho, mass = 100.0, (lambda x: 1.0 / (x * (1.0 + x) ** 3)), (lambda x: (x / (1.0 + x)) ** 2)
+    elif model == "nfw":
+        rmax, rho, mass = 10.0, (lambda x: 1.0 / (x * (1.0 + x) ** 2)), _nfw_mu
+    else:
+        raise ValueError(f"no velocity recipe for {model}")
+    grid = np.geomspace(1e-6, rmax, 4096)
+    f = rho(grid) * (mass(grid) / mass(rmax)) / grid ** 2
+    seg = 0.5 * (f[1:] + f[:-1]) * np.diff(grid)
+    tail = np.concatenate([np.cumsum(seg[::-1])[::-1], [0.0]])           # int_r^rmax
+    sigma2 = tail / rho(grid)
+    sig = np.sqrt(np.interp(np.clip(r, grid[0], rmax), grid, sigma2))
+    rng = _rng(seed)
+    vel = np.zeros((pos_m.shape[0], 4), np.float32)
+    vel[:, :3] = (rng.normal(size=(pos_m.shape[0], 3)) * sig[:, None]).astype(np.float32)
+    return vel
+
+
 def random_active_subset(n: int, fraction: float, seed: int = 7) -> np.ndarray:
     """Ascending uint32 indices of a random subset (BASELINE.json configs[4], fixed seed)."""
     rng = _rng(seed)
@@ -167,6 +193,27 @@ CONFIGS = {
     "m31_2p24_block": dict(model=m31_like, n=1 << 24, eps=2.0 ** -8, delta_acc=2.0 ** -9, block=True, r_crit=0.5, group_size=32),
     "nfw_2p22_sweep": dict(model=nfw, n=1 << 22, eps=2.0 ** -8, delta_acc=2.0 ** -9, block=False, r_crit=0.5, group_size=32),
 }
+
+
+# Live block-stepping runs (moving particles): the same spheres with isotropic_velocities(); not BASELINE.json configs
+# (those carry no velocities) but the workloads of the time-to-solution measurement SURVEY.md 8f row 1 asks for.
+LIVE_CONFIGS = {
+    "plummer_2p20_live": dict(model="plummer", n=1 << 20, eps=2.0 ** -7, delta_acc=2.0 ** -9, r_crit=1.0, group_size=32),
+    "nfw_2p22_live": dict(model="nfw", n=1 << 22, eps=2.0 ** -8, delta_acc=2.0 ** -9, r_crit=0.5, group_size=32),
+    "nfw_2p24_live": dict(model="nfw", n=1 << 24, eps=2.0 ** -8, delta_acc=2.0 ** -9, r_crit=0.5, group_size=32),
+}
+
+
+def make_live_config(name: str, seed: int = 1, n: int | None = None) -> tuple[np.ndarray, np.ndarray, dict]:
+    """Returns (pos_m float32 [N,4], vel float32 [N,4], parameters) of a live block-stepping workload."""
+    cfg = dict(LIVE_CONFIGS[name])
+    if n is not None:
+        cfg["n"] = int(n)
+    pos = globals()[cfg["model"]](cfg["n"], seed)
+    vel = isotropic_velocities(pos, cfg["model"], seed + 1000)
+    cfg["name"] = name
+    cfg["seed"] = seed
+    return pos, vel, cfg
 
 
 def make_config(name: str, seed: int = 1, n: int | None = None) -> tuple[np.ndarray, dict]:
