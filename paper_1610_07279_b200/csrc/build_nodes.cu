@@ -265,6 +265,11 @@ int gothic_stage_nodes(gothic_ctx *c, uint32_t n, int n_leaf, cudaStream_t s)
     GOTHIC_CUDA_OK(c, cudaMemcpyAsync(c->h_level_ofs, c->level_ofs, (GOTHIC_NLEVP1 + 1) * sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
     GOTHIC_CUDA_OK(c, cudaMemcpyAsync(h_flags, c->flags, sizeof(h_flags), cudaMemcpyDeviceToHost, s));
     GOTHIC_CUDA_OK(c, cudaStreamSynchronize(s));
+    if (h_flags[3]) {       // the keys are not fully sorted: nothing above can be trusted (sort_pairs.cu, gothic_build_tree repeats the build)
+        GOTHIC_CUDA_OK(c, cudaMemsetAsync(c->flags + 3, 0, sizeof(uint32_t), s));
+        GOTHIC_CUDA_OK(c, cudaMemsetAsync(c->flags, 0, sizeof(uint32_t), s));
+        return GOTHIC_RETRY_FULL_SORT;
+    }
     if (h_flags[0]) return GOTHIC_ERR_CAPACITY;
     c->n_nodes = h_flags[2];
     c->n_levels_tree = 0;

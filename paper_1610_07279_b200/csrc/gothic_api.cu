@@ -171,10 +171,13 @@ int gothic_build_tree(gothic_ctx *c, const float *pos_m, uint32_t n, int key_kin
     c->n = n;
     c->n_leaf = n_leaf;
     int rc;
-    if ((rc = gothic_stage_keys(c, pos, n, key_kind, s)) != GOTHIC_OK) return rc;
-    if ((rc = gothic_stage_sort(c, n, s)) != GOTHIC_OK) return rc;
-    if ((rc = gothic_stage_gather(c, pos, n, s)) != GOTHIC_OK) return rc;
-    if ((rc = gothic_stage_nodes(c, n, n_leaf, s)) != GOTHIC_OK) return rc;
+    for (int full = 0; full < 2; full++) {      // second round only if the five-pass sort met a long unordered run (sort_pairs.cu)
+        if ((rc = gothic_stage_keys(c, pos, n, key_kind, s)) != GOTHIC_OK) return rc;
+        if ((rc = gothic_stage_sort(c, n, full != 0, s)) != GOTHIC_OK) return rc;
+        if ((rc = gothic_stage_gather(c, pos, n, s)) != GOTHIC_OK) return rc;
+        if ((rc = gothic_stage_nodes(c, n, n_leaf, s)) != GOTHIC_RETRY_FULL_SORT) break;
+    }
+    if (rc != GOTHIC_OK) return rc == GOTHIC_RETRY_FULL_SORT ? GOTHIC_ERR_STATE : rc;
     if ((rc = gothic_stage_moments(c, s)) != GOTHIC_OK) return rc;
     c->built = true;
     return GOTHIC_OK;

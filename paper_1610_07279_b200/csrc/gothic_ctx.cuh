@@ -61,7 +61,7 @@ struct gothic_ctx {
     uint32_t *level_cnt;   // [22]
     uint32_t *blk_cnt;     // [2][22][nblk_max] per-block start/end event counts
     uint32_t nblk_max;
-    uint32_t *flags;       // [4]: 0 = capacity overflow (nodes), 1 = stack overflow, 2 = n_nodes, 3 = spare
+    uint32_t *flags;       // [4]: 0 = capacity overflow (nodes), 1 = stack overflow, 2 = n_nodes, 3 = the fast sort needs the full passes
     // sort scratch
     void *sort_tmp;
     size_t sort_tmp_bytes;
@@ -99,7 +99,8 @@ void gothic_live_free(gothic_ctx *c);
 
 // ---- stage entry points (each in its own .cu) --------------------------------------------------------
 int gothic_stage_keys(gothic_ctx *c, const float4 *pos_m, uint32_t n, int key_kind, cudaStream_t s);
-int gothic_stage_sort(gothic_ctx *c, uint32_t n, cudaStream_t s);
+int gothic_stage_sort(gothic_ctx *c, uint32_t n, bool full, cudaStream_t s);   // full = all 8 digit passes (the retry of gothic_build_tree)
+#define GOTHIC_RETRY_FULL_SORT 1     // internal return of gothic_stage_nodes: the fast sort left a long run unordered (flags[3])
 size_t gothic_sort_scratch_bytes(uint32_t n_max);
 int gothic_keys_config(gothic_ctx *c);     // uploads the Peano-Hilbert state table (called by gothic_create)
 cudaError_t gothic_sort_config();         // per-device function attributes of the sort kernels (called by gothic_create)

@@ -13,12 +13,25 @@
 // Per pass every pair is read once and written once (12 B each way): the HBM floor of an LSD radix sort.  Ties keep
 // ascending original index (LSD passes are stable), which is what makes perm bit-exact against the oracle's
 // std::stable_sort.
+//
+// Five passes instead of eight.  The low 23 bits of a key (the last 7 2/3 octal digits: cells of 2^-13.3 of the root cube) order
+// particles only inside runs of equal upper 40 bits, and such runs are short (most particles are alone in theirs).  So the LSD
+// passes cover bits 23..62 only, and
+//   k_sort_fix_short  finds the runs and finishes the ones of up to 32 keys by a stable insertion sort on the low bits (one thread
+//                     per run; nothing to do when the run is already in order, e.g. coincident particles),
+//   k_sort_fix_long   finishes runs of 33 .. FIX_LONG_MAX keys by a stable rank sort in shared memory (one CTA per run).
+// A longer run that is out of order raises flags[3]; gothic_build_tree then repeats the build with all eight passes (a pathological
+// input: thousands of distinct particles inside one cell of 2^-13 of the box).
 #include "gothic_ctx.cuh"
 
 namespace {
 
 constexpr int RADIX = 256;
-constexpr int NPASS = 8;                    // 8 x 8 bits >= 63
+constexpr int NPASS = 8;                    // 8 x 8 bits >= 63 (the full sort; the fast path runs the upper NPASS_FAST digits)
+constexpr int NPASS_FAST = 5;
+constexpr int LOW_BITS = 63 - 8 * NPASS_FAST;          // 23 bits left to the fix-up kernels
+constexpr int FIX_SHORT_MAX = 32;
+constexpr int FIX_LONG_MAX = 2048;
 constexpr int SORT_TPB = 256;
 constexpr int SORT_WARPS = SORT_TPB / 32;
 #ifndef GOTHIC_SORT_IPT
@@ -37,16 +50,17 @@ constexpr uint32_t FULL = 0xffffffffu;
 // scratch layout (u32 words): ghist[NPASS][RADIX] | ticket[NPASS] (+ pad to 16) | status[NPASS][ntiles][RADIX]
 __host__ __device__ inline size_t sort_words_head() { return (size_t)NPASS * RADIX + 16; }
 
-__global__ void __launch_bounds__(SORT_TPB) k_sort_hist(const uint64_t *__restrict__ key, uint32_t n, uint32_t *__restrict__ ghist)
+__global__ void __launch_bounds__(SORT_TPB) k_sort_hist(const uint64_t *__restrict__ key, uint32_t n, uint32_t *__restrict__ ghist, int shift0, int npass)
 {
     __shared__ uint32_t s_h[NPASS][RADIX];
     for (int i = threadIdx.x; i < NPASS * RADIX; i += SORT_TPB) (&s_h[0][0])[i] = 0u;
     __syncthreads();
     const uint32_t stride = gridDim.x * SORT_TPB;
     for (uint32_t i = blockIdx.x * SORT_TPB + threadIdx.x; i < n; i += stride) {
-        const uint64_t k = __ldg(key + i);
+        const uint64_t k = __ldg(key + i) >> shift0;
 #pragma unroll
-        for (int p = 0; p < NPASS; p++) atomicAdd(&s_h[p][(uint32_t)(k >> (8 * p)) & 255u], 1u);
+        for (int p = 0; p < NPASS; p++)
+            if (p < npass) atomicAdd(&s_h[p][(uint32_t)(k >> (8 * p)) & 255u], 1u);
     }
     __syncthreads();
     for (int i = threadIdx.x; i < NPASS * RADIX; i += SORT_TPB) {
@@ -197,12 +211,74 @@ __global__ void __launch_bounds__(SORT_TPB, GOTHIC_SORT_CTAS) k_sort_onesweep(co
     }
 }
 
+// Runs of equal upper bits (key >> LOW_BITS) after the fast passes: inside a run the keys are in ascending original index and
+// still have to be ordered by their low bits, stably.  One thread per run start; runs that are already in order cost one scan.
+__global__ void __launch_bounds__(SORT_TPB) k_sort_fix_short(uint64_t *__restrict__ key, uint32_t *__restrict__ val, uint32_t n,
+                                                              uint2 *__restrict__ long_runs, uint32_t long_cap, uint32_t *__restrict__ n_long,
+                                                              uint32_t *__restrict__ flags)
+{
+    const uint32_t i = blockIdx.x * SORT_TPB + threadIdx.x;
+    if (i >= n) return;
+    const uint64_t ki = key[i];
+    const uint64_t top = ki >> LOW_BITS;
+    if (i > 0 && (key[i - 1] >> LOW_BITS) == top) return;          // not the first of its run
+    if (i + 1 >= n || (key[i + 1] >> LOW_BITS) != top) return;      // a run of one
+    uint32_t len = 1;
+    bool ordered = true;
+    uint64_t prev = ki;
+    while (i + len < n) {
+        const uint64_t kj = key[i + len];
+        if ((kj >> LOW_BITS) != top) break;
+        ordered = ordered && prev <= kj;
+        prev = kj;
+        len++;
+    }
+    if (ordered) return;
+    if (len <= (uint32_t)FIX_SHORT_MAX) {
+        for (uint32_t a = 1; a < len; a++) {                       // stable insertion sort: an entry passes strictly larger keys only
+            const uint64_t k = key[i + a];
+            const uint32_t v = val[i + a];
+            uint32_t b = a;
+            while (b > 0 && key[i + b - 1] > k) { key[i + b] = key[i + b - 1]; val[i + b] = val[i + b - 1]; b--; }
+            key[i + b] = k; val[i + b] = v;
+        }
+    } else if (len <= (uint32_t)FIX_LONG_MAX) {
+        const uint32_t at = atomicAdd(n_long, 1u);
+        if (at < long_cap) long_runs[at] = make_uint2(i, len);
+        else atomicExch(flags + 3, 1u);
+    } else atomicExch(flags + 3, 1u);
+}
+
+// One CTA per long run: rank of an entry = number of entries with a smaller key, or with an equal key and an earlier place.
+__global__ void __launch_bounds__(SORT_TPB) k_sort_fix_long(uint64_t *__restrict__ key, uint32_t *__restrict__ val, const uint2 *__restrict__ long_runs,
+                                                             uint32_t long_cap, const uint32_t *__restrict__ n_long)
+{
+    __shared__ uint64_t sk[FIX_LONG_MAX];
+    __shared__ uint32_t sv[FIX_LONG_MAX];
+    const uint32_t n_runs = min(*n_long, long_cap);
+    for (uint32_t r = blockIdx.x; r < n_runs; r += gridDim.x) {
+        const uint2 run = long_runs[r];
+        for (uint32_t e = threadIdx.x; e < run.y; e += SORT_TPB) { sk[e] = key[run.x + e]; sv[e] = val[run.x + e]; }
+        __syncthreads();
+        for (uint32_t e = threadIdx.x; e < run.y; e += SORT_TPB) {
+            const uint64_t k = sk[e];
+            uint32_t rank = 0;
+            for (uint32_t j = 0; j < run.y; j++) rank += (sk[j] < k || (sk[j] == k && j < e)) ? 1u : 0u;
+            key[run.x + rank] = k;
+            val[run.x + rank] = sv[e];
+        }
+        __syncthreads();
+    }
+}
+
 } // namespace
+
+static size_t sort_long_cap(uint32_t n_max) { return (size_t)n_max / (FIX_SHORT_MAX + 1) + 1; }
 
 size_t gothic_sort_scratch_bytes(uint32_t n_max)
 {
     const size_t ntiles = ((size_t)n_max + TILE - 1) / TILE;
-    return (sort_words_head() + (size_t)NPASS * ntiles * RADIX) * sizeof(uint32_t);
+    return (sort_words_head() + (size_t)NPASS * ntiles * RADIX + 2 * sort_long_cap(n_max) + 4) * sizeof(uint32_t);
 }
 
 cudaError_t gothic_sort_config()
@@ -212,24 +288,35 @@ cudaError_t gothic_sort_config()
     return e;
 }
 
-int gothic_stage_sort(gothic_ctx *c, uint32_t n, cudaStream_t s)
+int gothic_stage_sort(gothic_ctx *c, uint32_t n, bool full, cudaStream_t s)
 {
-    const uint32_t ntiles = (n + TILE - 1) / TILE;
+    const uint32_t ntiles = (n + TILE - 1) / TILE, ntiles_max = (c->n_max + TILE - 1) / TILE;
     uint32_t *words = static_cast<uint32_t *>(c->sort_tmp);
     uint32_t *ghist = words, *ticket = words + NPASS * RADIX, *status = words + sort_words_head();
+    uint32_t *n_long = status + (size_t)NPASS * ntiles_max * RADIX;
+    uint2 *long_runs = reinterpret_cast<uint2 *>(n_long + 4);
+    const int npass = full ? NPASS : NPASS_FAST, shift0 = full ? 0 : LOW_BITS;
     GOTHIC_CUDA_OK(c, cudaMemsetAsync(words, 0, (sort_words_head() + (size_t)NPASS * ntiles * RADIX) * sizeof(uint32_t), s));
     int grid = (int)((n + SORT_TPB - 1) / SORT_TPB);
     if (grid > c->num_sms * 8) grid = c->num_sms * 8;
-    k_sort_hist<<<grid, SORT_TPB, 0, s>>>(c->key[c->cur], n, ghist);
+    k_sort_hist<<<grid, SORT_TPB, 0, s>>>(c->key[c->cur], n, ghist, shift0, npass);
     GOTHIC_LAUNCH_OK(c);
-    k_sort_scan<<<NPASS, RADIX, 0, s>>>(ghist);
+    k_sort_scan<<<npass, RADIX, 0, s>>>(ghist);
     GOTHIC_LAUNCH_OK(c);
-    for (int p = 0; p < NPASS; p++) {
+    for (int p = 0; p < npass; p++) {
         const int in = c->cur, out = c->cur ^ 1;
-        k_sort_onesweep<<<ntiles, SORT_TPB, sizeof(SortSmem), s>>>(c->key[in], p == 0 ? nullptr : c->idx[in], c->key[out], c->idx[out], n, 8 * p,
+        k_sort_onesweep<<<ntiles, SORT_TPB, sizeof(SortSmem), s>>>(c->key[in], p == 0 ? nullptr : c->idx[in], c->key[out], c->idx[out], n, shift0 + 8 * p,
                                                                     ghist + p * RADIX, ticket + p, status + (size_t)p * ntiles * RADIX);
         GOTHIC_LAUNCH_OK(c);
         c->cur = out;
+    }
+    if (!full) {
+        GOTHIC_CUDA_OK(c, cudaMemsetAsync(n_long, 0, sizeof(uint32_t), s));
+        const uint32_t long_cap = (uint32_t)sort_long_cap(c->n_max);
+        k_sort_fix_short<<<(n + SORT_TPB - 1) / SORT_TPB, SORT_TPB, 0, s>>>(c->key[c->cur], c->idx[c->cur], n, long_runs, long_cap, n_long, c->flags);
+        GOTHIC_LAUNCH_OK(c);
+        k_sort_fix_long<<<c->num_sms * 2, SORT_TPB, 0, s>>>(c->key[c->cur], c->idx[c->cur], long_runs, long_cap, n_long);
+        GOTHIC_LAUNCH_OK(c);
     }
     return GOTHIC_OK;
 }

@@ -54,6 +54,32 @@ def test_build_tiny_and_ragged(oracle, n):
     _check_build(oracle, W.plummer(n, seed=n), 0, 4)
 
 
+@pytest.mark.parametrize("n_clump,spread,kind", [(40, 1e-4, 0), (600, 3e-4, 0), (1500, 3e-4, 1), (5000, 2e-4, 0), (20000, 1e-5, 0)])
+def test_sort_runs_of_equal_upper_bits(oracle, n_clump, spread, kind):
+    """B3's five-pass sort leaves the low 23 key bits to fix-up kernels (sort_pairs.cu): a tight clump of DISTINCT particles inside one
+    cell of 2^-13 of a wide root cube gives runs of equal upper bits that are short (insertion sort), medium (rank sort in shared
+    memory) or too long for either (the build then repeats itself with all eight passes): perm must be the oracle's in every case."""
+    rng = np.random.default_rng(n_clump)
+    n_far = 3000
+    pos = np.zeros((n_far + 3 * n_clump, 4), np.float32)
+    pos[:n_far, :3] = rng.uniform(-16.0, 16.0, (n_far, 3))
+    for c, ctr in enumerate(((0.123, 0.456, -0.789), (5.0, -3.0, 2.0), (-7.77, 7.77, 0.01))):
+        sl = slice(n_far + c * n_clump, n_far + (c + 1) * n_clump)
+        pos[sl, :3] = np.asarray(ctr, np.float32) + rng.uniform(-spread, spread, (n_clump, 3)).astype(np.float32)
+    pos[:, 3] = 1.0 / pos.shape[0]
+    pos = pos[rng.permutation(pos.shape[0])]
+    from gpu_util import gpu_build
+    g, v = gpu_build(pos, key_kind=kind)
+    t = oracle.build_tree(pos, key_kind=kind)
+    assert np.array_equal(v["key"], t.key) and np.array_equal(v["perm"], t.perm) and np.array_equal(v["pos_m_sorted"], t.pos_sorted)
+    assert v["n_nodes"] == t.n_nodes and np.array_equal(v["node_head"], t.head) and np.array_equal(v["node_num"], t.num)
+    assert np.array_equal(v["node_child"], t.child) and np.array_equal(v["node_level"], t.level)
+    g.close()
+    top = t.key >> np.uint64(23)
+    runs = np.diff(np.flatnonzero(np.concatenate([[True], top[1:] != top[:-1], [True]])))
+    assert runs.max() >= min(n_clump // 8, 33) or n_clump < 100       # the case really has long runs of equal upper bits
+
+
 def test_build_degenerate_inputs(oracle):
     # all particles at one point: root cube side 1, one level-21 leaf chain
     pos = np.tile(np.array([[0.25, -1.0, 3.0, 0.01]], np.float32), (100, 1))
