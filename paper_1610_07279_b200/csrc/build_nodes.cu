@@ -9,6 +9,7 @@
 //               particles = max over windows [i, i+n_leaf] containing p of shared_digits(key[i], key[i+n_leaf])
 //   p STARTS a node at every level L in [delta(p)+1, min(D(p)+1, 21)]
 //   p ENDS   a node at every level L in [delta(p+1)+1, min(D(p)+1, 21)]
+//   (both ranges are what k_node_events stores per key, four bytes; k_emit_nodes reads them back instead of the keys)
 //
 // (a level-L run is a node iff its parent run has more than n_leaf particles, and run sizes shrink monotonically
 // with depth).  The k-th start and the k-th end of a level belong to the same node; node id = level offset +
@@ -20,49 +21,22 @@ namespace {
 
 constexpr int TPB = 256;
 constexpr int NW = TPB / 32;
+constexpr int IPT = 8;                                   // keys per thread in the two event passes
+constexpr int TILE = TPB * IPT;                          // keys per CTA (2048): key p of a tile sits in row q = (p - base) / TPB
+constexpr int NROW = IPT * NW;                           // (row, warp) pairs of a tile, in key order
 
-struct Events { int s_lo, s_hi, e_lo, e_hi; };
+constexpr int KEYS_SM = TILE + 2 * GOTHIC_MAX_NLEAF;    // keys base - H .. base + TILE + H
+constexpr int WIN_SM = TILE + GOTHIC_MAX_NLEAF;         // window values of positions base - H .. base + TILE
 
-constexpr int KEYS_SM = TPB + 2 * GOTHIC_MAX_NLEAF;     // keys blockbase - H .. blockbase + TPB + H
-constexpr int WIN_SM = TPB + GOTHIC_MAX_NLEAF;          // window values of positions blockbase - H .. blockbase + TPB
-
-// D(p) is a sliding-window maximum of w(i) = shared_digits(key[i], key[i + H]) over i in [p - H, p]: every w is
-// computed once, then the window maxima of widths 2, 4, 8, ... are built by doubling in shared memory.
-// sw0 / sw1: ping-pong arrays of WIN_SM entries.  Returns D for the thread's own particle.
-__device__ __forceinline__ int window_depth(const uint64_t *sk, int8_t *sw0, int8_t *sw1, uint32_t n, int H)
+// The four event levels of one key in one word: bytes (s_lo, s_hi, e_lo, e_hi); an empty range has lo > hi.
+__device__ __forceinline__ uint32_t pack_events(int s_lo, int s_hi, int e_lo, int e_hi)
 {
-    const long long g0 = (long long)blockIdx.x * TPB - H;          // particle index of window slot 0
-    const int len = TPB + H;
-    for (int t = threadIdx.x; t < len; t += TPB) {
-        const long long i = g0 + t;
-        sw0[t] = (i >= 0 && i + H < (long long)n) ? (int8_t)shared_digits(sk[t], sk[t + H]) : (int8_t)-1;
-    }
-    __syncthreads();
-    const int W = H + 1;                                            // window width
-    int8_t *cur = sw0, *nxt = sw1;
-    int k = 1;
-    while (2 * k <= W) {
-        for (int t = threadIdx.x; t + k < len; t += TPB) nxt[t] = max(cur[t], cur[t + k]);
-        for (int t = max(len - k, 0) + threadIdx.x; t < len; t += TPB) nxt[t] = cur[t];
-        __syncthreads();
-        int8_t *tmp = cur; cur = nxt; nxt = tmp;
-        k *= 2;
-    }
-    // cur[t] = max of w over slots [t, t + k); the thread's window is slots [tid, tid + W)
-    return max((int)cur[threadIdx.x], (int)cur[threadIdx.x + W - k]);
+    return (uint32_t)s_lo | ((uint32_t)s_hi << 8) | ((uint32_t)e_lo << 16) | ((uint32_t)e_hi << 24);
 }
-
-__device__ __forceinline__ Events node_events(const uint64_t *sk, int8_t *sw0, int8_t *sw1, int tid, uint32_t p, uint32_t n, int H)
+struct Events { int s_lo, s_hi, e_lo, e_hi; };
+__device__ __forceinline__ Events unpack_events(uint32_t w)
 {
-    const int D = window_depth(sk, sw0, sw1, n, H);
-    Events ev = {1, 0, 1, 0};
-    if (p < n) {
-        const uint64_t kp = sk[H + tid];
-        const int dprev = p == 0 ? -1 : shared_digits(sk[H + tid - 1], kp);
-        const int dnext = p == n - 1 ? -1 : shared_digits(kp, sk[H + tid + 1]);
-        const int top = min(D + 1, GOTHIC_NLEV);
-        ev.s_lo = dprev + 1; ev.s_hi = top; ev.e_lo = dnext + 1; ev.e_hi = top;
-    }
+    Events ev = {(int)(w & 255u), (int)((w >> 8) & 255u), (int)((w >> 16) & 255u), (int)(w >> 24)};
     return ev;
 }
 
@@ -77,39 +51,67 @@ __device__ __forceinline__ void warp_level_range(const Events &ev, int &lo, int 
     hi = __reduce_max_sync(0xffffffffu, h);
 }
 
-__device__ __forceinline__ void load_keys(uint64_t *sk, const uint64_t *__restrict__ key, uint32_t n, int H)
-{
-    const long long base = (long long)blockIdx.x * TPB - H;
-    for (int t = threadIdx.x; t < TPB + 2 * H; t += TPB) {
-        const long long g = base + t;
-        sk[t] = (g >= 0 && g < (long long)n) ? __ldg(key + g) : 0ull;
-    }
-    __syncthreads();
-}
-
-// blk_cnt layout: [kind(0 = start, 1 = end)][level][nblk]
-__global__ void __launch_bounds__(TPB) k_count_events(const uint64_t *__restrict__ key, uint32_t n, int H,
-                                                       uint32_t *__restrict__ blk_cnt, uint32_t nblk)
+// Pass 1: the events of every key, computed once and kept as one word per key, and their counts per (tile, level).
+// D(p) is a sliding-window maximum of w(i) = shared_digits(key[i], key[i + H]) over i in [p - H, p]: every w is computed once, then
+// the window maxima of widths 2, 4, 8, ... are built by doubling in shared memory.
+// blk_cnt layout: [kind(0 = start, 1 = end)][level][ntile]
+__global__ void __launch_bounds__(TPB) k_node_events(const uint64_t *__restrict__ key, uint32_t n, int H, uint32_t *__restrict__ events,
+                                                      uint32_t *__restrict__ blk_cnt, uint32_t ntile)
 {
     __shared__ uint64_t sk[KEYS_SM];
     __shared__ int8_t sw[2][WIN_SM];
     __shared__ uint32_t tot[2][GOTHIC_NLEVP1];
     if (threadIdx.x < 2 * GOTHIC_NLEVP1) (&tot[0][0])[threadIdx.x] = 0;
-    load_keys(sk, key, n, H);
-    const Events ev = node_events(sk, sw[0], sw[1], threadIdx.x, blockIdx.x * TPB + threadIdx.x, n, H);
-    int Llo, Lhi;
-    warp_level_range(ev, Llo, Lhi);
-    for (int L = Llo; L <= Lhi; L++) {
-        const uint32_t bs = __ballot_sync(0xffffffffu, ev.s_lo <= L && L <= ev.s_hi);
-        const uint32_t be = __ballot_sync(0xffffffffu, ev.e_lo <= L && L <= ev.e_hi);
-        if (lane_id() == 0) {
-            if (bs) atomicAdd(&tot[0][L], __popc(bs));
-            if (be) atomicAdd(&tot[1][L], __popc(be));
+    const long long base = (long long)blockIdx.x * TILE;
+    for (int t = threadIdx.x; t < TILE + 2 * H; t += TPB) {
+        const long long g = base - H + t;
+        sk[t] = (g >= 0 && g < (long long)n) ? __ldg(key + g) : 0ull;
+    }
+    __syncthreads();
+    const int len = TILE + H;
+    for (int t = threadIdx.x; t < len; t += TPB) {
+        const long long i = base - H + t;
+        sw[0][t] = (i >= 0 && i + H < (long long)n) ? (int8_t)shared_digits(sk[t], sk[t + H]) : (int8_t)-1;
+    }
+    __syncthreads();
+    const int W = H + 1;                                            // window width
+    int8_t *cur = sw[0], *nxt = sw[1];
+    int k = 1;
+    while (2 * k <= W) {
+        for (int t = threadIdx.x; t < len; t += TPB) nxt[t] = t + k < len ? max(cur[t], cur[t + k]) : cur[t];
+        __syncthreads();
+        int8_t *tmp = cur; cur = nxt; nxt = tmp;
+        k *= 2;
+    }
+    // cur[t] = max of w over slots [t, t + k); the window of key base + j is slots [j, j + W)
+#pragma unroll
+    for (int q = 0; q < IPT; q++) {
+        const int j = q * TPB + threadIdx.x;
+        const long long p = base + j;
+        Events ev = {1, 0, 1, 0};
+        if (p < (long long)n) {
+            const int D = max((int)cur[j], (int)cur[j + W - k]);
+            const uint64_t kp = sk[H + j];
+            const int dprev = p == 0 ? -1 : shared_digits(sk[H + j - 1], kp);
+            const int dnext = p == (long long)n - 1 ? -1 : shared_digits(kp, sk[H + j + 1]);
+            const int top = min(D + 1, GOTHIC_NLEV);
+            ev.s_lo = dprev + 1; ev.s_hi = top; ev.e_lo = dnext + 1; ev.e_hi = top;
+            events[p] = pack_events(ev.s_lo, ev.s_hi, ev.e_lo, ev.e_hi);
+        }
+        int Llo, Lhi;
+        warp_level_range(ev, Llo, Lhi);
+        for (int L = Llo; L <= Lhi; L++) {
+            const uint32_t bs = __ballot_sync(0xffffffffu, ev.s_lo <= L && L <= ev.s_hi);
+            const uint32_t be = __ballot_sync(0xffffffffu, ev.e_lo <= L && L <= ev.e_hi);
+            if (lane_id() == 0) {
+                if (bs) atomicAdd(&tot[0][L], __popc(bs));
+                if (be) atomicAdd(&tot[1][L], __popc(be));
+            }
         }
     }
     __syncthreads();
     if (threadIdx.x < 2 * GOTHIC_NLEVP1)
-        blk_cnt[(size_t)threadIdx.x * nblk + blockIdx.x] = (&tot[0][0])[threadIdx.x];
+        blk_cnt[(size_t)threadIdx.x * ntile + blockIdx.x] = (&tot[0][0])[threadIdx.x];
 }
 
 // One block per (kind, level): exclusive scan over blocks in place; totals of the start rows -> level_cnt.
@@ -165,55 +167,67 @@ __global__ void k_level_offsets(const uint32_t *level_cnt, uint32_t *level_ofs, 
     if (acc > node_max) flags[0] = 1u;
 }
 
-__global__ void __launch_bounds__(TPB) k_emit_nodes(const uint64_t *__restrict__ key, uint32_t n, int H,
-                                                     const uint32_t *__restrict__ blk_cnt, uint32_t nblk,
+// Pass 2: node ids from the scanned counts, node arrays written.  Reads the event words of pass 1 (4 bytes per key), not the keys.
+__global__ void __launch_bounds__(TPB) k_emit_nodes(const uint32_t *__restrict__ events, uint32_t n,
+                                                     const uint32_t *__restrict__ blk_cnt, uint32_t ntile,
                                                      const uint32_t *__restrict__ level_ofs, const uint32_t *__restrict__ flags,
                                                      uint32_t *__restrict__ node_head, uint8_t *__restrict__ node_level,
                                                      uint32_t *__restrict__ node_child, uint32_t *__restrict__ node_end,
                                                      uint32_t *__restrict__ node_last)
 {
-    __shared__ uint64_t sk[KEYS_SM];
-    __shared__ int8_t sw[2][WIN_SM];
-    __shared__ uint32_t wcnt[2][GOTHIC_NLEVP1][NW];   // per-warp counts -> exclusive prefix + block base + level offset
+    __shared__ uint32_t wcnt[2][GOTHIC_NLEVP1][NROW];   // counts per (row, warp) in key order -> exclusive prefix + tile base + level offset
     if (flags[0]) return;
-    for (int t = threadIdx.x; t < 2 * GOTHIC_NLEVP1 * NW; t += TPB) (&wcnt[0][0][0])[t] = 0u;
-    load_keys(sk, key, n, H);
-    const uint32_t p = blockIdx.x * TPB + threadIdx.x;
-    const Events ev = node_events(sk, sw[0], sw[1], threadIdx.x, p, n, H);
+    for (int t = threadIdx.x; t < 2 * GOTHIC_NLEVP1 * NROW; t += TPB) (&wcnt[0][0][0])[t] = 0u;
+    const uint32_t base = blockIdx.x * (uint32_t)TILE;
     const int warp = threadIdx.x >> 5;
-    int Llo, Lhi;
-    warp_level_range(ev, Llo, Lhi);
-    for (int L = Llo; L <= Lhi; L++) {
-        const uint32_t bs = __ballot_sync(0xffffffffu, ev.s_lo <= L && L <= ev.s_hi);
-        const uint32_t be = __ballot_sync(0xffffffffu, ev.e_lo <= L && L <= ev.e_hi);
-        if (lane_id() == 0) { wcnt[0][L][warp] = __popc(bs); wcnt[1][L][warp] = __popc(be); }
+    Events ev[IPT];
+#pragma unroll
+    for (int q = 0; q < IPT; q++) {
+        const uint32_t p = base + q * TPB + threadIdx.x;
+        ev[q] = unpack_events(p < n ? __ldg(events + p) : pack_events(1, 0, 1, 0));
+    }
+    __syncthreads();
+#pragma unroll
+    for (int q = 0; q < IPT; q++) {
+        int Llo, Lhi;
+        warp_level_range(ev[q], Llo, Lhi);
+        for (int L = Llo; L <= Lhi; L++) {
+            const uint32_t bs = __ballot_sync(0xffffffffu, ev[q].s_lo <= L && L <= ev[q].s_hi);
+            const uint32_t be = __ballot_sync(0xffffffffu, ev[q].e_lo <= L && L <= ev[q].e_hi);
+            if (lane_id() == 0) { wcnt[0][L][q * NW + warp] = __popc(bs); wcnt[1][L][q * NW + warp] = __popc(be); }
+        }
     }
     __syncthreads();
     if (threadIdx.x < 2 * GOTHIC_NLEVP1) {
         const int kind = threadIdx.x / GOTHIC_NLEVP1, L = threadIdx.x % GOTHIC_NLEVP1;
-        uint32_t run = level_ofs[L] + blk_cnt[(size_t)threadIdx.x * nblk + blockIdx.x];
-#pragma unroll
-        for (int w = 0; w < NW; w++) { const uint32_t c = wcnt[kind][L][w]; wcnt[kind][L][w] = run; run += c; }
+        uint32_t run = level_ofs[L] + blk_cnt[(size_t)threadIdx.x * ntile + blockIdx.x];
+        for (int w = 0; w < NROW; w++) { const uint32_t c = wcnt[kind][L][w]; wcnt[kind][L][w] = run; run += c; }
     }
     __syncthreads();
     const uint32_t lt = (1u << lane_id()) - 1u;
-    uint32_t sid_below = GOTHIC_LEAF, eid_below = GOTHIC_LEAF;   // ids of this thread's events one level deeper
-    for (int L = Lhi; L >= Llo; L--) {
-        const bool fs = ev.s_lo <= L && L <= ev.s_hi, fe = ev.e_lo <= L && L <= ev.e_hi;
-        const uint32_t bs = __ballot_sync(0xffffffffu, fs);
-        const uint32_t be = __ballot_sync(0xffffffffu, fe);
-        if (fs) {
-            const uint32_t id = wcnt[0][L][warp] + __popc(bs & lt);
-            node_head[id] = p;
-            node_level[id] = (uint8_t)L;
-            node_child[id] = (L + 1 <= ev.s_hi) ? sid_below : GOTHIC_LEAF;
-            sid_below = id;
-        }
-        if (fe) {
-            const uint32_t id = wcnt[1][L][warp] + __popc(be & lt);
-            node_end[id] = p + 1;
-            node_last[id] = (L + 1 <= ev.e_hi) ? eid_below : GOTHIC_LEAF;
-            eid_below = id;
+#pragma unroll
+    for (int q = 0; q < IPT; q++) {
+        const uint32_t p = base + q * TPB + threadIdx.x;
+        int Llo, Lhi;
+        warp_level_range(ev[q], Llo, Lhi);
+        uint32_t sid_below = GOTHIC_LEAF, eid_below = GOTHIC_LEAF;   // ids of this key's events one level deeper
+        for (int L = Lhi; L >= Llo; L--) {
+            const bool fs = ev[q].s_lo <= L && L <= ev[q].s_hi, fe = ev[q].e_lo <= L && L <= ev[q].e_hi;
+            const uint32_t bs = __ballot_sync(0xffffffffu, fs);
+            const uint32_t be = __ballot_sync(0xffffffffu, fe);
+            if (fs) {
+                const uint32_t id = wcnt[0][L][q * NW + warp] + __popc(bs & lt);
+                node_head[id] = p;
+                node_level[id] = (uint8_t)L;
+                node_child[id] = (L + 1 <= ev[q].s_hi) ? sid_below : GOTHIC_LEAF;
+                sid_below = id;
+            }
+            if (fe) {
+                const uint32_t id = wcnt[1][L][q * NW + warp] + __popc(be & lt);
+                node_end[id] = p + 1;
+                node_last[id] = (L + 1 <= ev[q].e_hi) ? eid_below : GOTHIC_LEAF;
+                eid_below = id;
+            }
         }
     }
 }
@@ -247,17 +261,18 @@ __global__ void __launch_bounds__(TPB) k_finish_nodes(uint32_t n_nodes, const ui
 
 int gothic_stage_nodes(gothic_ctx *c, uint32_t n, int n_leaf, cudaStream_t s)
 {
-    const uint32_t nblk = (n + TPB - 1) / TPB;
+    const uint32_t nblk = (n + TILE - 1) / TILE;
     const uint64_t *key = c->key[c->cur];
+    uint32_t *events = c->leaf_of;          // one word per key between the two passes; k_finish_nodes then overwrites it with the leaf ids
     // only the build's own overflow flag: flags[1] (the walk's stack overflow) stays set until gothic_check reads it, flags[2] is rewritten below
     GOTHIC_CUDA_OK(c, cudaMemsetAsync(c->flags, 0, sizeof(uint32_t), s));
-    k_count_events<<<nblk, TPB, 0, s>>>(key, n, n_leaf, c->blk_cnt, nblk);
+    k_node_events<<<nblk, TPB, 0, s>>>(key, n, n_leaf, events, c->blk_cnt, nblk);
     GOTHIC_LAUNCH_OK(c);
     k_scan_blocks<<<2 * GOTHIC_NLEVP1, SCAN_TPB, 0, s>>>(c->blk_cnt, nblk, c->level_cnt);
     GOTHIC_LAUNCH_OK(c);
     k_level_offsets<<<1, 1, 0, s>>>(c->level_cnt, c->level_ofs, c->flags, c->node_max);
     GOTHIC_LAUNCH_OK(c);
-    k_emit_nodes<<<nblk, TPB, 0, s>>>(key, n, n_leaf, c->blk_cnt, nblk, c->level_ofs, c->flags, c->node_head, c->node_level,
+    k_emit_nodes<<<nblk, TPB, 0, s>>>(events, n, c->blk_cnt, nblk, c->level_ofs, c->flags, c->node_head, c->node_level,
                                       c->node_child, c->node_end, c->node_last);
     GOTHIC_LAUNCH_OK(c);
     // the one host read of the build: node count + level offsets (sizes the remaining launches)
