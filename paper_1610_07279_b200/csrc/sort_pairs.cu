@@ -173,12 +173,20 @@ __global__ void __launch_bounds__(SORT_TPB, GOTHIC_SORT_CTAS) k_sort_onesweep(co
         // decoupled look-back: sum of this digit's counts over tiles tile-1, tile-2, ... until an inclusive one
         uint32_t prefix = 0;
         if (tile > 0) {
-            uint32_t t = tile - 1;
-            for (;;) {
-                const uint32_t s = status[(size_t)t * RADIX + tid];
-                if (s & ST_INC) { prefix += s & ST_VAL; break; }
-                if (s & ST_AGG) { prefix += s & ST_VAL; t--; continue; }
-                __nanosleep(20);
+            // four earlier tiles per step: their status words are independent loads, so a step costs one L2 round trip, not four
+            int t = (int)tile - 1;
+            bool done = false;
+            while (!done) {
+                uint32_t sw[4];
+#pragma unroll
+                for (int q = 0; q < 4; q++) sw[q] = t - q >= 0 ? status[(size_t)(t - q) * RADIX + tid] : 0x80000000u;
+#pragma unroll
+                for (int q = 0; q < 4; q++) {
+                    if (done) break;
+                    if (sw[q] & ST_INC) { prefix += sw[q] & ST_VAL; done = true; }
+                    else if (sw[q] & ST_AGG) { prefix += sw[q] & ST_VAL; t--; }
+                    else { __nanosleep(20); break; }        // not published yet: look again from this tile
+                }
             }
             *st = (prefix + count) | ST_INC;
         }
