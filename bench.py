@@ -472,7 +472,7 @@ def measure_live(torch, W, B, workload: str, *, seed: int, n, dev, alu_peak: flo
         def run_cycle(counter=None, log=None):
             st = g.live_get(arrays=False)
             for s in range(st["n_substeps"]):
-                rebuild = (s == 0) if k == "cycle" else (st["steps"] + s) % k == 0
+                rebuild = (s == 0) if k == "cycle" else (st["steps"] + s + 1) % k == 0      # the k-th step of every k: with k = 2, 4 the even (populous) substeps get the fresh tree
                 g.live_step(delta_acc=dacc, r_crit=r_crit, rebuild=rebuild, n_interactions=counter)
                 if log is not None:
                     now = g.live_get(arrays="n_active")
