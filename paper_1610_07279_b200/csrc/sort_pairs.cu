@@ -132,7 +132,14 @@ __global__ void __launch_bounds__(SORT_TPB, GOTHIC_SORT_CTAS) k_sort_onesweep(co
         const uint32_t j = warp * (32u * IPT) + (uint32_t)i * 32u + lane;
         const bool valid = j < n_valid;
         const uint32_t d = (uint32_t)(k[i] >> shift) & 255u;
-        const uint32_t peers = __match_any_sync(FULL, valid ? d : 256u);
+        // the lanes of the row with the same digit: eight ballots (one per digit bit) instead of match.any, which is the slower of the two here
+        uint32_t peers = __ballot_sync(FULL, valid);
+        if (!valid) peers = ~peers;
+#pragma unroll
+        for (int b = 0; b < 8; b++) {
+            const uint32_t vote = __ballot_sync(FULL, (d >> b) & 1u);
+            peers &= ((d >> b) & 1u) ? vote : ~vote;
+        }
         const int leader = __ffs(peers) - 1;
         // one returning shared-memory atomic per distinct digit of the row: atomics of one warp on one address complete in
         // program order, so the rows need no barrier between them and their latencies overlap
