@@ -3,7 +3,7 @@
 //
 //   k_sort_hist      one pass over the keys -> the 8 digit histograms (8 bits per digit, 63 significant bits),
 //   k_sort_scan      exclusive scan of each histogram = where every digit's run starts in the output of its pass,
-//   k_sort_onesweep  one launch per digit, least significant first.  A CTA takes the next tile of 4096 pairs (ticket
+//   k_sort_onesweep  one launch per digit, least significant first.  A CTA takes the next tile of 3072 pairs (ticket
 //                    from an atomic counter, so that every earlier tile is already running), ranks its keys by
 //                    digit (warp-private counters + match.any, items in index order => stable), publishes its digit
 //                    counts, finds the sum over all earlier tiles by decoupled look-back (each of the 256 threads
@@ -35,13 +35,13 @@ constexpr int FIX_LONG_MAX = 2048;
 constexpr int SORT_TPB = 256;
 constexpr int SORT_WARPS = SORT_TPB / 32;
 #ifndef GOTHIC_SORT_IPT
-#define GOTHIC_SORT_IPT 16
+#define GOTHIC_SORT_IPT 12
 #endif
 #ifndef GOTHIC_SORT_CTAS
-#define GOTHIC_SORT_CTAS 3
+#define GOTHIC_SORT_CTAS 4
 #endif
 constexpr int IPT = GOTHIC_SORT_IPT;        // items per thread
-constexpr int TILE = SORT_TPB * IPT;        // pairs per CTA (4096)
+constexpr int TILE = SORT_TPB * IPT;        // pairs per CTA (3072: four CTAs of 256 threads per SM)
 constexpr uint32_t ST_AGG = 1u << 30;       // status word: this tile's own count is in the low 30 bits
 constexpr uint32_t ST_INC = 1u << 31;       //              the count of this and ALL earlier tiles is
 constexpr uint32_t ST_VAL = ST_AGG - 1u;
