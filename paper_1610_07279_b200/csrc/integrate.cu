@@ -234,7 +234,7 @@ int gothic_live_step(gothic_ctx *c, float delta_acc, float r_crit, int rebuild, 
 {
     if (!c || !(delta_acc >= 0.0f) || !(r_crit >= 0.0f)) return GOTHIC_ERR_ARG;
     gothic_live *L = c->live;
-    if (!L || !c->built) return GOTHIC_ERR_STATE;
+    if (!L || !c->built || c->n != L->n) return GOTHIC_ERR_STATE;     // (a gothic_build_tree of another particle set in between ends the live run)
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const uint32_t n = L->n, grid = (n + TPB - 1) / TPB;
     const float dt_unit = ldexpf(1.0f, L->e_min);

@@ -134,9 +134,29 @@ def study_balls(n: int):
     g.close()
 
 
+def study_sort(n: int):
+    """The library comparison VERDICT r01 asked to state next to B3: torch.sort(stable=True) (CUB's radix sort of 64-bit keys, with 64-bit
+    indices as payload) on the workload's own keys in their pre-sort order, against the whole gothic_build_tree (keys + sort + gather +
+    nodes + moments) of the same particles.  Context only: nothing of the library links or calls it."""
+    pos_np, cfg = W.make_config("nfw_2p24_block", seed=1, n=n)
+    g = Gothic(n)
+    pos = torch.from_numpy(pos_np).cuda()
+    g.build_tree(pos)
+    v = g.get_tree_view()
+    inv = torch.empty(n, dtype=torch.int64, device="cuda")
+    inv[v["perm"].long()] = torch.arange(n, device="cuda")
+    keys_unsorted = v["key"][inv].contiguous()              # key of original particle i
+    ms_torch = _timed(lambda: torch.sort(keys_unsorted, stable=True), reps=5)
+    ms_build = _timed(lambda: g.build_tree(pos), reps=5)
+    srt, idx = torch.sort(keys_unsorted, stable=True)
+    same = bool(torch.equal(idx.int(), v["perm"])) and bool(torch.equal(srt, v["key"]))
+    print(json.dumps({"study": "sort", "n": n, "torch_sort_stable_ms": ms_torch, "gothic_build_tree_ms": ms_build, "same_permutation": same}), flush=True)
+    g.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("study", choices=["keys", "refresh", "balls"])
+    ap.add_argument("study", choices=["keys", "refresh", "balls", "sort"])
     ap.add_argument("--n", type=int, default=1 << 22)
     ap.add_argument("--steps", type=int, default=32)
     a = ap.parse_args()
@@ -144,6 +164,8 @@ def main():
         study_keys(a.n)
     elif a.study == "refresh":
         study_refresh(min(a.n, 1 << 20), a.steps)
+    elif a.study == "sort":
+        study_sort(a.n)
     else:
         study_balls(a.n)
 
