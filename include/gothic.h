@@ -41,7 +41,7 @@ enum {
 };
 
 enum { GOTHIC_KEY_PEANO_HILBERT = 0, GOTHIC_KEY_MORTON = 1 };   /* PAPER.md:54 / PAPER.md:564 */
-enum { GOTHIC_BALL_GEO = 0, GOTHIC_BALL_EBS = 1, GOTHIC_BALL_COM = 2, GOTHIC_BALL_CMP = 3 };   /* enclosing ball of an i-group, App. B PAPER.md:568 items 3, 2, 4, 5 */
+enum { GOTHIC_BALL_GEO = 0, GOTHIC_BALL_EBS = 1, GOTHIC_BALL_COM = 2, GOTHIC_BALL_CMP = 3, GOTHIC_BALL_SEB = 4 };   /* enclosing ball of an i-group, App. B PAPER.md:568 items 3, 2, 4, 5, 1 */
 enum { GOTHIC_MAC_ACCELERATION = 0, GOTHIC_MAC_OPENING_ANGLE = 1, GOTHIC_MAC_MULTIPOLE = 2 }; /* eq. 5 PAPER.md:85-89 / eq. 2 PAPER.md:68-72 / eq. 3-4 */
 
 /* Allocates a context for up to n_max particles (n_max <= 2^30: the sort's look-back words carry 30-bit prefixes).
@@ -161,7 +161,8 @@ int gothic_block_cycle_host(gothic_ctx *ctx, const float *pos_m_host, const floa
 
 /* Enclosing ball of the pseudo i-particle used by the following walks (App. B): GOTHIC_BALL_GEO (default;
  * centre of the members' bounding cuboid), GOTHIC_BALL_EBS (Ritter's efficient bounding sphere; R17), GOTHIC_BALL_COM
- * (centre of mass of the members) or GOTHIC_BALL_CMP (the smaller of GEO and COM).  In all of them the
+ * (centre of mass of the members), GOTHIC_BALL_CMP (the smaller of GEO and COM) or GOTHIC_BALL_SEB (the smallest enclosing ball, by Welzl's
+ * move-to-front recursion in single precision, R19; the costliest generator, PAPER.md:568 Table B.4).  In all of them the
  * radius is the exact maximum distance of the members from the centre.  Also decides the r_crit splitting (R13). */
 int gothic_set_ball(gothic_ctx *ctx, int ball_kind);
 

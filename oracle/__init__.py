@@ -269,7 +269,7 @@ def walk_tree(t: Tree, **kw):
 
 
 def group_ball(pos_sorted, members, ball_kind: int = 0) -> np.ndarray:
-    """(r_I, b_I) as the walk forms it: ball_kind 0 = GEO, 1 = EBS (Ritter), App. B P:568."""
+    """(r_I, b_I) as the walk forms it: ball_kind 0 = GEO, 1 = EBS (Ritter), 2 = COM, 3 = CMP, 4 = SEB (smallest enclosing ball), App. B P:568."""
     out = np.zeros(4, np.float32)
     members = np.ascontiguousarray(members, np.uint32)
     lib().oracle_group_ball(_pos(pos_sorted), members, members.shape[0], int(ball_kind), out)

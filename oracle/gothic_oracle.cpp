@@ -385,11 +385,98 @@ static float ball_radius2(const float *pos_sorted, const uint32_t *members, uint
     return b2max;
 }
 
+/*   ball_kind 4, SEB (item 1): the smallest enclosing ball.  The paper names Fischer et al. (2003) and gives nothing else; the ball
+ *     itself is unique, so any exact method serves.  Reading R19: Welzl's move-to-front recursion over the members in ascending
+ *     order, single precision, operations as written.  A support set of m <= 4 points fixes the ball through them (m = 1 the point,
+ *     2 the midpoint, 3 the circumcircle's centre in their plane, 4 the circumsphere: Cramer's rule about the first support point);
+ *     a (near-)degenerate set (determinant <= 1e-12 of its scale) keeps the ball of the set without its last point.  A member counts
+ *     as outside when its squared distance exceeds r^2 (1 + 2^-20).  As for the other balls the radius used by the walk is then the
+ *     exact maximum distance of the members from the centre found, so rounding can cost tightness, never enclosure. */
+struct SebBall { float c[3]; float r2; };
+
+static SebBall seb_from_support(const float S[4][3], int m)
+{
+    SebBall B;
+    B.c[0] = B.c[1] = B.c[2] = 0.0f;
+    B.r2 = -1.0f;
+    if (m == 0) return B;
+    if (m == 1) { B.c[0] = S[0][0]; B.c[1] = S[0][1]; B.c[2] = S[0][2]; B.r2 = 0.0f; return B; }
+    if (m == 2) {
+        for (int d = 0; d < 3; d++) B.c[d] = 0.5f * (S[0][d] + S[1][d]);
+        B.r2 = dist2f(S[0], B.c);
+        return B;
+    }
+    const float a[3] = {S[1][0] - S[0][0], S[1][1] - S[0][1], S[1][2] - S[0][2]};
+    const float b[3] = {S[2][0] - S[0][0], S[2][1] - S[0][1], S[2][2] - S[0][2]};
+    const float aa = fmaf(a[2], a[2], fmaf(a[1], a[1], a[0] * a[0]));
+    const float bb = fmaf(b[2], b[2], fmaf(b[1], b[1], b[0] * b[0]));
+    const float ab = fmaf(a[2], b[2], fmaf(a[1], b[1], a[0] * b[0]));
+    if (m == 3) {
+        const float det = fmaf(aa, bb, -(ab * ab));
+        if (!(det > 1e-12f * (aa * bb))) return seb_from_support(S, 2);
+        const float l1 = (0.5f * (bb * (aa - ab))) / det, l2 = (0.5f * (aa * (bb - ab))) / det;
+        float x[3];
+        for (int d = 0; d < 3; d++) x[d] = fmaf(l2, b[d], l1 * a[d]);
+        for (int d = 0; d < 3; d++) B.c[d] = S[0][d] + x[d];
+        B.r2 = fmaf(x[2], x[2], fmaf(x[1], x[1], x[0] * x[0]));
+        return B;
+    }
+    const float c[3] = {S[3][0] - S[0][0], S[3][1] - S[0][1], S[3][2] - S[0][2]};
+    const float cc = fmaf(c[2], c[2], fmaf(c[1], c[1], c[0] * c[0]));
+    /* b x c, c x a, a x b */
+    const float bc[3] = {fmaf(b[1], c[2], -(b[2] * c[1])), fmaf(b[2], c[0], -(b[0] * c[2])), fmaf(b[0], c[1], -(b[1] * c[0]))};
+    const float ca[3] = {fmaf(c[1], a[2], -(c[2] * a[1])), fmaf(c[2], a[0], -(c[0] * a[2])), fmaf(c[0], a[1], -(c[1] * a[0]))};
+    const float axb[3] = {fmaf(a[1], b[2], -(a[2] * b[1])), fmaf(a[2], b[0], -(a[0] * b[2])), fmaf(a[0], b[1], -(a[1] * b[0]))};
+    const float det = fmaf(a[2], bc[2], fmaf(a[1], bc[1], a[0] * bc[0]));
+    if (!(fabsf(det) > 1e-12f * sqrtf(aa * bb * cc))) return seb_from_support(S, 3);
+    const float h = 0.5f / det;
+    float x[3];
+    for (int d = 0; d < 3; d++) x[d] = h * fmaf(cc, axb[d], fmaf(bb, ca[d], aa * bc[d]));
+    for (int d = 0; d < 3; d++) B.c[d] = S[0][d] + x[d];
+    B.r2 = fmaf(x[2], x[2], fmaf(x[1], x[1], x[0] * x[0]));
+    return B;
+}
+
+/* Welzl: smallest ball of pts[idx[0 .. n)] with the m points of S on its boundary; idx is reordered (move to front). */
+static SebBall seb_mtf(const float (*pts)[3], uint8_t *idx, int n, float S[4][3], int m, int *budget)
+{
+    SebBall B = seb_from_support(S, m);
+    if (m == 4) return B;
+    for (int i = 0; i < n; i++) {
+        const float *p = pts[idx[i]];
+        if (B.r2 < 0.0f || dist2f(p, B.c) > B.r2 * (1.0f + 9.5367431640625e-07f)) {
+            if (--(*budget) < 0) return B;                       /* cannot happen for points in general position */
+            S[m][0] = p[0]; S[m][1] = p[1]; S[m][2] = p[2];
+            B = seb_mtf(pts, idx, i, S, m + 1, budget);
+            const uint8_t t = idx[i];
+            for (int j = i; j > 0; j--) idx[j] = idx[j - 1];
+            idx[0] = t;
+        }
+    }
+    return B;
+}
+
+static void seb_centre(const float *pos_sorted, const uint32_t *members, uint32_t k, float rI[3])
+{
+    float pts[64][3];
+    uint8_t idx[64];
+    const int n = (int)std::min<uint32_t>(k, 64u);
+    for (int q = 0; q < n; q++) {
+        for (int d = 0; d < 3; d++) pts[q][d] = pos_sorted[4 * (size_t)members[q] + d];
+        idx[q] = (uint8_t)q;
+    }
+    float S[4][3];
+    int budget = 4096;
+    const SebBall B = seb_mtf(pts, idx, n, S, 0, &budget);
+    rI[0] = B.c[0]; rI[1] = B.c[1]; rI[2] = B.c[2];
+}
+
 /*   ball_kind 2, COM (item 4): centre of mass of the members, sums over the members in ascending order with one fmaf each, then
  *     one division per coordinate.
  *   ball_kind 3, CMP (item 5): the smaller of the GEO and COM balls (GEO on ties). */
 static void ball_centre(const float *pos_sorted, const uint32_t *members, uint32_t k, int ball_kind, float rI[3])
 {
+    if (ball_kind == 4) { seb_centre(pos_sorted, members, k, rI); return; }
     if (ball_kind == 2 || ball_kind == 3) {
         float sx = 0.0f, sy = 0.0f, sz = 0.0f, sm = 0.0f;
         for (uint32_t q = 0; q < k; q++) {

@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libgothic_b200.so")
 
 KEY_PEANO_HILBERT, KEY_MORTON = 0, 1
 MAC_ACCELERATION, MAC_OPENING_ANGLE, MAC_MULTIPOLE = 0, 1, 2
-BALL_GEO, BALL_EBS, BALL_COM, BALL_CMP = 0, 1, 2, 3
+BALL_GEO, BALL_EBS, BALL_COM, BALL_CMP, BALL_SEB = 0, 1, 2, 3, 4
 
 EXPORTS = [
     "gothic_create", "gothic_destroy", "gothic_strerror", "gothic_last_cuda_error", "gothic_build_tree",

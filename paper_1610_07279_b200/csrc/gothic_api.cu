@@ -152,7 +152,7 @@ void gothic_destroy(gothic_ctx *ctx)
 
 int gothic_set_ball(gothic_ctx *ctx, int ball_kind)
 {
-    if (!ctx || (ball_kind < GOTHIC_BALL_GEO || ball_kind > GOTHIC_BALL_CMP)) return GOTHIC_ERR_ARG;
+    if (!ctx || (ball_kind < GOTHIC_BALL_GEO || ball_kind > GOTHIC_BALL_SEB)) return GOTHIC_ERR_ARG;
     ctx->ball_kind = ball_kind;
     return GOTHIC_OK;
 }

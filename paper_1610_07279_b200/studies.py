@@ -17,7 +17,7 @@ import numpy as np
 import torch
 
 from . import workloads as W
-from .binding import BALL_CMP, BALL_COM, BALL_EBS, BALL_GEO, KEY_MORTON, KEY_PEANO_HILBERT, MAC_ACCELERATION, MAC_MULTIPOLE, MAC_OPENING_ANGLE, Gothic
+from .binding import BALL_CMP, BALL_COM, BALL_EBS, BALL_GEO, BALL_SEB, KEY_MORTON, KEY_PEANO_HILBERT, MAC_ACCELERATION, MAC_MULTIPOLE, MAC_OPENING_ANGLE, Gothic
 
 
 def _timed(fn, reps=3):
@@ -121,7 +121,7 @@ def study_balls(n: int):
     ref = torch.zeros(n, 4, device="cuda")
     g.walk_tree(ref, eps=eps, mac_kind=MAC_OPENING_ANGLE, mac_param=0.5, amag_out=amag)
     g.walk_tree(ref, eps=eps, mac_kind=MAC_ACCELERATION, mac_param=2.0 ** -22, aold=amag)        # tight walk as the yardstick
-    for ball_name, ball in (("GEO", BALL_GEO), ("EBS", BALL_EBS), ("COM", BALL_COM), ("CMP", BALL_CMP)):
+    for ball_name, ball in (("GEO", BALL_GEO), ("EBS", BALL_EBS), ("COM", BALL_COM), ("CMP", BALL_CMP), ("SEB", BALL_SEB)):
         g.set_ball(ball)
         for mac_name, mac, params in (("acceleration", MAC_ACCELERATION, [2.0 ** -e for e in (5, 7, 9, 11)]),
                                       ("multipole", MAC_MULTIPOLE, [2.0 ** -e for e in (0, 3, 6, 9)]),

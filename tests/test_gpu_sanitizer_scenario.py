@@ -49,7 +49,7 @@ def test_scenario_all_kernels(oracle, G):
     sparse = W.random_active_subset(n, 0.07, seed=3)
     # every MAC x every ball, full and sparse active sets, with and without group splitting
     for mac_kind, param in ((0, 2.0 ** -8), (1, 0.55), (2, 2.0 ** -6)):
-        for ball in (0, 1, 2, 3):
+        for ball in (0, 1, 2, 3, 4):
             g.set_ball(ball)
             for act, r_crit in ((None, float("inf")), (sparse, 0.2), (act_ref, 0.0)):
                 _, cnt, _ = gpu_walk(g, n, eps=eps, mac_kind=mac_kind, mac_param=param, aold=aold, active=act, r_crit=r_crit)

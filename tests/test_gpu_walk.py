@@ -277,7 +277,7 @@ def test_walk_ebs_ball_matches_oracle(oracle, model, n, G, frac, r_crit):
         assert cnt == c["interactions"]
         _assert_parity(out, ref, rows)
         counts[kind] = cnt
-    for ball in (2, 3):         # COM and CMP (App. B items 4 and 5)
+    for ball in (2, 3, 4):      # COM, CMP and SEB (App. B items 4, 5 and 1)
         g.set_ball(ball)
         out, cnt, _ = gpu_walk(g, n, eps=eps, mac_kind=0, mac_param=2.0 ** -8, aold=aold, active=active, r_crit=r_crit)
         ref, c = _oracle_on_gpu_tree(oracle, v, eps=eps, mac_kind=0, mac_param=2.0 ** -8, aold=aold, active=active, group_size=G,
@@ -350,7 +350,7 @@ def test_walk_randomised_parity_sweep(oracle):
         active = None if frac == 1.0 else W.random_active_subset(n, frac, seed=it)
         rows = np.arange(n) if active is None else active
         r_crit = float(rng.choice([np.inf, 1.0, 0.3, 0.05, 0.0]))
-        ball = int(rng.integers(0, 4))          # GEO, EBS, COM, CMP
+        ball = int(rng.integers(0, 5))          # GEO, EBS, COM, CMP, SEB
         g.set_ball(ball)
         kind = int(rng.integers(0, 3))
         param = {0: 2.0 ** -float(rng.integers(4, 18)), 1: float(rng.uniform(0.15, 0.9)), 2: 2.0 ** -float(rng.integers(0, 16))}[kind]

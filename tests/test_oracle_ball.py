@@ -25,7 +25,7 @@ def _seb_radius(x, iters=4000):
 def test_members_are_enclosed_and_radius_is_the_exact_maximum():
     rng = np.random.default_rng(1)
     for k in (1, 2, 3, 5, 17, 32):
-        for kind in (0, 1, 2, 3):
+        for kind in (0, 1, 2, 3, 4):
             p = _pts(k, rng, scale=10.0 ** rng.uniform(-3, 1))
             ball = oracle.group_ball(p, np.arange(k), kind)
             d = np.sqrt(((p[:, :3].astype(np.float64) - ball[:3].astype(np.float64)) ** 2).sum(1))
@@ -38,7 +38,7 @@ def test_special_cases():
     two = np.array([[0, 0, 0, 1], [2, 4, 4, 1]], np.float32)                       # distance 6
     line = np.zeros((9, 4), np.float32)
     line[:, 0] = np.arange(9)                                                      # collinear: diameter 8
-    for kind in (0, 1, 2, 3):
+    for kind in (0, 1, 2, 3, 4):
         b = oracle.group_ball(one, [0], kind)
         assert np.array_equal(b[:3], one[0, :3]) and b[3] == 0
         b = oracle.group_ball(two, [0, 1], kind)
@@ -49,7 +49,7 @@ def test_special_cases():
     rng = np.random.default_rng(2)
     p = _pts(40, rng)
     mem = np.array([3, 7, 8, 20, 31], np.uint32)
-    for kind in (0, 1, 2, 3):
+    for kind in (0, 1, 2, 3, 4):
         assert np.array_equal(oracle.group_ball(p, mem, kind), oracle.group_ball(p[mem], np.arange(5), kind))
 
 
@@ -90,3 +90,47 @@ def test_com_and_cmp_balls():
     p = _pts(6, rng)
     p[:, 3] = 0.0
     assert np.array_equal(oracle.group_ball(p, np.arange(6), 2), oracle.group_ball(p, np.arange(6), 0))
+
+
+def _seb_by_definition(x):
+    """The smallest enclosing ball written out (double): it is fixed by 2, 3 or 4 of the points on its boundary, so the smallest ball
+    among the circumscribed balls of all such subsets that contain every point is it.  O(k^4): tiny sets only."""
+    from itertools import combinations
+    k = x.shape[0]
+    best = (np.inf, None)
+    for m in (2, 3, 4):
+        for sub in combinations(range(k), m):
+            q = x[list(sub)]
+            a = q[1:] - q[0]                                   # centre = q0 + sum l_j a_j, 2 a_i . (c - q0) = |a_i|^2
+            g = 2.0 * a @ a.T
+            if abs(np.linalg.det(g)) < 1e-14 * np.prod(np.diag(g)):
+                continue
+            lam = np.linalg.solve(g, (a * a).sum(1))
+            c = q[0] + lam @ a
+            r = np.sqrt(((q[0] - c) ** 2).sum())
+            if r < best[0] and np.all(np.sqrt(((x - c) ** 2).sum(1)) <= r * (1 + 1e-9)):
+                best = (r, c)
+    return best
+
+
+def test_seb_is_the_smallest_enclosing_ball():
+    """App. B item 1: the oracle's SEB (Welzl's recursion in single precision, reading R19) against the definition in double on
+    random sets of 2 .. 12 points, on points of a sphere's surface (many near-cospherical supports) and on flat and collinear sets."""
+    rng = np.random.default_rng(11)
+    cases = [_pts(int(rng.integers(2, 13)), rng, scale=10.0 ** rng.uniform(-2, 1)) for _ in range(60)]
+    sph = rng.normal(size=(10, 3)); sph /= np.linalg.norm(sph, axis=1)[:, None]
+    p = np.zeros((10, 4), np.float32); p[:, :3] = 3.0 * sph + 1.0; cases.append(p)
+    flat = _pts(9, rng); flat[:, 2] = 0.5; cases.append(flat)
+    for p in cases:
+        k = p.shape[0]
+        r_def, c_def = _seb_by_definition(p[:, :3].astype(np.float64))
+        b = oracle.group_ball(p, np.arange(k), 4)
+        assert r_def * (1 - 1e-6) <= b[3] <= r_def * (1 + 2e-5), (k, b[3], r_def)
+        assert np.linalg.norm(b[:3] - c_def) <= 3e-3 * r_def
+    # and it is never larger than the other generators' balls (Fig. B.10 plots r_ball / r_SEB >= 1)
+    for _ in range(200):
+        k = int(rng.integers(2, 33))
+        p = _pts(k, rng)
+        r = [oracle.group_ball(p, np.arange(k), kind)[3] for kind in (0, 1, 2, 3, 4)]
+        assert r[4] <= min(r[:4]) * (1 + 1e-5)
+        assert r[4] >= _seb_radius(p[:, :3].astype(np.float64)) * (1 - 2e-3)
