@@ -235,19 +235,13 @@ __global__ void __launch_bounds__(TPB) k_emit_nodes(const uint32_t *__restrict__
 __global__ void __launch_bounds__(TPB) k_finish_nodes(uint32_t n_nodes, const uint32_t *__restrict__ node_head,
                                                        const uint32_t *__restrict__ node_end, const uint32_t *__restrict__ node_child,
                                                        const uint32_t *__restrict__ node_last, uint32_t *__restrict__ node_num,
-                                                       uint8_t *__restrict__ node_nchild, uint32_t *__restrict__ node_parent, uint32_t *__restrict__ leaf_of,
-                                                       const uint8_t *__restrict__ node_level, uint8_t *__restrict__ leaf_level)
+                                                       uint8_t *__restrict__ node_nchild, uint32_t *__restrict__ node_parent)
 {
     const uint32_t J = blockIdx.x * TPB + threadIdx.x;
     if (J >= n_nodes) return;
     const uint32_t h = node_head[J], num = node_end[J] - h;
     node_num[J] = num;
     const uint32_t c = node_child[J];
-    if (c == GOTHIC_LEAF)
-    {
-        const uint8_t lv = node_level[J];
-        for (uint32_t i = 0; i < num; i++) { leaf_of[h + i] = J; leaf_level[h + i] = lv; }
-    }
     uint32_t nc = 0;
     if (c != GOTHIC_LEAF) {
         nc = node_last[J] - c + 1u;
@@ -255,6 +249,19 @@ __global__ void __launch_bounds__(TPB) k_finish_nodes(uint32_t n_nodes, const ui
     }
     node_nchild[J] = (uint8_t)nc;
     if (J == 0) node_parent[0] = GOTHIC_LEAF;
+}
+
+// leaf_of / leaf_level of a particle: the PARENT of its leaf and that parent's level, which is where the radius climb of moments.cu starts
+// (a leaf's own radius comes out of k_leaf_moments).  After k_finish_nodes, which writes the parent links.
+__global__ void __launch_bounds__(TPB) k_leaf_links(uint32_t n_nodes, const uint32_t *__restrict__ node_head, const uint32_t *__restrict__ node_num,
+                                                     const uint32_t *__restrict__ node_child, const uint32_t *__restrict__ node_parent,
+                                                     const uint8_t *__restrict__ node_level, uint32_t *__restrict__ leaf_of, uint8_t *__restrict__ leaf_level)
+{
+    const uint32_t J = blockIdx.x * TPB + threadIdx.x;
+    if (J >= n_nodes || node_child[J] != GOTHIC_LEAF) return;
+    const uint32_t h = node_head[J], num = node_num[J], P = node_parent[J];
+    const uint8_t lv = P == GOTHIC_LEAF ? (uint8_t)0xFFu : node_level[P];       // the tree is one leaf: nothing to climb
+    for (uint32_t i = 0; i < num; i++) { leaf_of[h + i] = P; leaf_level[h + i] = lv; }
 }
 
 } // namespace
@@ -291,7 +298,10 @@ int gothic_stage_nodes(gothic_ctx *c, uint32_t n, int n_leaf, cudaStream_t s)
     for (int L = 0; L < GOTHIC_NLEVP1; L++)
         if (c->h_level_ofs[L + 1] > c->h_level_ofs[L]) c->n_levels_tree = L + 1;
     k_finish_nodes<<<(c->n_nodes + TPB - 1) / TPB, TPB, 0, s>>>(c->n_nodes, c->node_head, c->node_end, c->node_child, c->node_last,
-                                                                c->node_num, c->node_nchild, c->node_parent, c->leaf_of, c->node_level, c->leaf_level);
+                                                                c->node_num, c->node_nchild, c->node_parent);
+    GOTHIC_LAUNCH_OK(c);
+    k_leaf_links<<<(c->n_nodes + TPB - 1) / TPB, TPB, 0, s>>>(c->n_nodes, c->node_head, c->node_num, c->node_child, c->node_parent, c->node_level,
+                                                              c->leaf_of, c->leaf_level);
     GOTHIC_LAUNCH_OK(c);
     return GOTHIC_OK;
 }

@@ -17,11 +17,12 @@ namespace {
 constexpr int TPB = 256;
 
 __device__ __forceinline__ void store_com(uint32_t J, float4 ms, float4 com, float4 *__restrict__ node_msum, float4 *__restrict__ node_com,
-                                          uint32_t *__restrict__ node_b2bits, const uint32_t *__restrict__ node_parent, float4 *__restrict__ node_up)
+                                          uint32_t *__restrict__ node_b2bits, const uint32_t *__restrict__ node_parent, float4 *__restrict__ node_up,
+                                          uint32_t b2bits = 0u)
 {
     node_msum[J] = ms;
     node_com[J] = com;
-    node_b2bits[J] = 0u;
+    node_b2bits[J] = b2bits;
     node_up[J] = make_float4(com.x, com.y, com.z, __uint_as_float(node_parent[J]));
 }
 __device__ __forceinline__ float4 com_of(float4 ms)
@@ -49,7 +50,15 @@ __global__ void __launch_bounds__(TPB) k_leaf_moments(uint32_t n_nodes, const fl
         ms.x = fmaf(p.w, p.x, ms.x); ms.y = fmaf(p.w, p.y, ms.y); ms.z = fmaf(p.w, p.z, ms.z); ms.w += p.w;
     }
     const float4 cm = com_of(ms);
-    store_com(J, ms, cm, node_msum, node_com, node_b2bits, node_parent, node_up);
+    // the leaf's own radius (exact maximum, same arithmetic as k_node_radius): the radius climb then starts at the leaf's parent and
+    // is spared its most fragmented level
+    float b2 = 0.0f;
+    for (uint32_t j = h; j < h + c; j++) {
+        const float4 p = __ldg(pos + j);
+        const float dx = __fsub_rn(p.x, cm.x), dy = __fsub_rn(p.y, cm.y), dz = __fsub_rn(p.z, cm.z);
+        b2 = fmaxf(b2, fmaf(dz, dz, fmaf(dy, dy, __fmul_rn(dx, dx))));
+    }
+    store_com(J, ms, cm, node_msum, node_com, node_b2bits, node_parent, node_up, __float_as_uint(b2));
     if (!node_B2) return;
     float B2 = 0.0f;                                     // eq. 4 about the stored centre
     for (uint32_t j = h; j < h + c; j++) {
@@ -112,8 +121,8 @@ __global__ void __launch_bounds__(TPB) k_node_radius(uint32_t n, uint32_t per_wa
     uint32_t A_nx = GOTHIC_LEAF;
     int lev_nx = -1;
     if ((uint32_t)r0 + lane < r1) {
-        p_nx = __ldg(pos + (uint32_t)r0 + lane); A_nx = __ldg(leaf_of + (uint32_t)r0 + lane); lev_nx = __ldg(leaf_level + (uint32_t)r0 + lane);
-        u_nx = node_up[A_nx];
+        p_nx = __ldg(pos + (uint32_t)r0 + lane); A_nx = __ldg(leaf_of + (uint32_t)r0 + lane); lev_nx = (int)(int8_t)__ldg(leaf_level + (uint32_t)r0 + lane);
+        if (A_nx != GOTHIC_LEAF) u_nx = node_up[A_nx];
     }
     for (uint32_t s0 = (uint32_t)r0; s0 < r1; s0 += 32u) {
         const uint32_t s = s0 + lane;
@@ -122,7 +131,7 @@ __global__ void __launch_bounds__(TPB) k_node_radius(uint32_t n, uint32_t per_wa
         uint32_t A = A_nx;
         int lev = lev_nx;
         p_nx = make_float4(0.f, 0.f, 0.f, 0.f); A_nx = GOTHIC_LEAF; lev_nx = -1;
-        if (s + 32u < r1) { p_nx = __ldg(pos + s + 32u); A_nx = __ldg(leaf_of + s + 32u); lev_nx = __ldg(leaf_level + s + 32u); }
+        if (s + 32u < r1) { p_nx = __ldg(pos + s + 32u); A_nx = __ldg(leaf_of + s + 32u); lev_nx = (int)(int8_t)__ldg(leaf_level + s + 32u); }
         // ---- top-down over the levels whose remembered node contains the whole chunk (nested, so levels 0 .. Lf-1) ----
         const uint32_t in_mask = __ballot_sync(0xffffffffu, m_node != GOTHIC_LEAF && s0 >= m_head && min(s0 + 32u, r1) <= m_end);
         const int Lf = __ffs(~in_mask) - 1;
