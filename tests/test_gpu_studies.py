@@ -35,7 +35,10 @@ def test_balls_study(capsys):
     from paper_1610_07279_b200 import studies
     studies.study_balls(1 << 15)
     rows = _lines(capsys)
-    assert len(rows) == 48          # 4 balls x 3 MACs x 4 parameters
+    assert len(rows) == 60          # 5 balls x 3 MACs x 4 parameters
     for mac in ("acceleration", "multipole", "opening_angle"):
         geo = [d for d in rows if d["ball"] == "GEO" and d["mac"] == mac]
         assert all(b["err_median"] < a["err_median"] and b["interactions"] > a["interactions"] for a, b in zip(geo, geo[1:]))
+    # the smallest ball opens the fewest cells (App. B: "the best choice is the SEB, which has the minimum radius")
+    for a, b in zip([d for d in rows if d["ball"] == "SEB" and d["mac"] == "acceleration"], [d for d in rows if d["ball"] == "GEO" and d["mac"] == "acceleration"]):
+        assert a["param"] == b["param"] and a["interactions"] <= b["interactions"]
