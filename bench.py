@@ -183,7 +183,11 @@ def run_reference(args, rank: int, world: int):
     import oracle
     from paper_1610_07279_b200 import workloads as W
     t0 = time.time()
-    pos, cfg = W.make_config(args.workload, seed=args.seed, n=args.n)
+    if args.workload.endswith("_live"):      # the live workloads' spheres at their initial positions: the oracle walks one block cycle's active sets
+        pos, _, cfg = W.make_live_config(args.workload, seed=args.seed, n=args.n)
+        cfg["block"] = True
+    else:
+        pos, cfg = W.make_config(args.workload, seed=args.seed, n=args.n)
     n, eps, dacc = cfg["n"], cfg["eps"], cfg["delta_acc"]
     r_crit = cfg["r_crit"] if args.r_crit is None else args.r_crit
     t_gen = time.time() - t0
