@@ -1,9 +1,21 @@
 """Pins for the oracle's predictor-corrector (O8; eq. 15-17) against what the mathematics fixes:
 closed-form kinematics under a constant acceleration, the leap-frog it must reduce to for shared fixed steps,
 second-order convergence on the harmonic oscillator, and the block-alignment invariant of the level migration (R15)."""
+import math
+
 import numpy as np
 
 import oracle
+
+
+def _wanted_level(a_vec, eps, eta, e_min, max_levels):
+    """R6 written out in double with math.log2 (not through oracle.levels): the level the criterion dt = eta sqrt(eps/|a|), floored
+    to a power of two, asks for, and whether |a| sits so close to a power-of-two boundary of dt that single precision may round
+    to the other side."""
+    a = math.sqrt(sum(float(x) ** 2 for x in a_vec))
+    lg = math.log2(eta * math.sqrt(eps / a))
+    near = abs(lg - round(lg)) < 1e-3
+    return min(max(math.floor(lg) - e_min, 0), max_levels - 1), near
 
 
 def _state(n, rng):
@@ -100,6 +112,7 @@ def test_level_migration_keeps_blocks_aligned():
     pos, vel = _state(n, rng)
     t_last = np.zeros(n, np.uint32)
     unit = 2.0 ** e_min
+    saw_far_jump = False
     for t in range(1, 2 ** (max_levels - 1) + 1):
         active = oracle.active_set(level, t)
         assert np.all(t % (1 << level[active].astype(np.int64)) == 0)
@@ -115,4 +128,45 @@ def test_level_migration_keeps_blocks_aligned():
         coarser = active[moved[active] == 1]
         assert np.all(t % (1 << level[coarser].astype(np.int64)) == 0)
         assert np.all(level < max_levels)
+        # no corrected particle keeps a step longer than the criterion allows for its NEW acceleration (R6):
+        # finer is taken at once and in full, whatever the distance; coarser at most one level
+        jumps = 0
+        for i in active:
+            want, near = _wanted_level(acc_new[i, :3], eps, eta, e_min, max_levels)
+            if near:
+                continue
+            assert level[i] <= want, (t, i, before[i], level[i], want)
+            if want < before[i]:
+                assert level[i] == want, (t, i, before[i], level[i], want)
+                jumps += before[i] - want >= 2
+        saw_far_jump = saw_far_jump or jumps > 0
+    assert saw_far_jump                                   # the run did contain moves of two or more levels finer
     assert np.all(t_last[oracle.active_set(level, 2 ** (max_levels - 1))] <= 2 ** (max_levels - 1))
+
+
+def test_finer_migration_takes_the_whole_jump_at_once():
+    """Hand case for R15's "any FINER level at once": eps = 2^-8, eta = 1/2, |a| = 2^-8 / s^2 gives dt = s/2; with s = 1.5 * 2^j
+    that is 0.75 * 2^j, exponent j - 1, far from any boundary.  e_min = -10.  Particles on level 5 (j = -4) and level 3 (j = -6)
+    whose new |a| is 16x / 256x the old one (dt 4x / 16x shorter) must land exactly two / four levels finer in ONE correction,
+    clamped at level 0; one whose |a| falls 4x (dt 2x longer) goes one level coarser because t_now = 32 is a multiple of it."""
+    eps, eta, e_min, max_levels = 2.0 ** -8, 0.5, -10, 8
+    amag = lambda j: 2.0 ** -8 / (1.5 * 2.0 ** j) ** 2
+    cur = np.array([5, 5, 3, 3, 3], np.uint8)
+    scale = np.array([16.0, 256.0, 16.0, 256.0, 0.25])
+    expect = np.array([3, 1, 1, 0, 4], np.uint8)
+    n = cur.shape[0]
+    acc = np.zeros((n, 4), np.float32)
+    acc_new = np.zeros((n, 4), np.float32)
+    for i in range(n):
+        acc[i, i % 3] = amag(int(cur[i]) + e_min + 1)
+        acc_new[i, (i + 1) % 3] = -acc[i, i % 3] * scale[i]
+        assert _wanted_level(acc[i, :3], eps, eta, e_min, max_levels) == (cur[i], False)
+    t_now = 32
+    t_last = (t_now - (1 << cur.astype(np.int64))).astype(np.uint32)
+    rng = np.random.default_rng(9)
+    pos, vel = _state(n, rng)
+    level = cur.copy()
+    pred = oracle.predict(pos, vel, acc, t_last, t_now, 2.0 ** e_min)
+    oracle.correct(np.arange(n, dtype=np.uint32), pred, acc_new, t_now, 2.0 ** e_min, pos, vel, acc, t_last, level,
+                   eps=eps, eta=eta, e_min=e_min, max_levels=max_levels)
+    assert level.tolist() == expect.tolist()
