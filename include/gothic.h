@@ -37,7 +37,8 @@ enum {
     GOTHIC_ERR_STATE = -2,         /* walk / update before a successful build */
     GOTHIC_ERR_CAPACITY = -3,      /* node pool or traversal stack overflow */
     GOTHIC_ERR_CUDA = -4,          /* CUDA runtime error (see gothic_last_cuda_error) */
-    GOTHIC_ERR_UNIMPLEMENTED = -5
+    GOTHIC_ERR_UNIMPLEMENTED = -5,
+    GOTHIC_ERR_TOO_LARGE = -6      /* gothic_active_list_static: n above GOTHIC_STATIC_ACTIVE_MAX_N */
 };
 
 enum { GOTHIC_KEY_PEANO_HILBERT = 0, GOTHIC_KEY_MORTON = 1 };   /* PAPER.md:54 / PAPER.md:564 */
@@ -229,6 +230,40 @@ int gothic_live_init(gothic_ctx *ctx, const float *pos_m, const float *vel, uint
                      float eta, int max_levels, float theta_boot, void *stream);
 int gothic_live_step(gothic_ctx *ctx, float delta_acc, float r_crit, int rebuild, unsigned long long *n_interactions, void *stream);
 int gothic_live_get(gothic_ctx *ctx, gothic_live_state *out);
+
+/* Active list of one substep for callers that must not allocate device memory.
+ *
+ * Who this is for.  Every other compute call needs a gothic_ctx, and gothic_create sizes and cudaMallocs its buffers.  That does
+ * not suit a host program that took the GPU's memory for itself at start-up -- an N-body code whose particle arrays are sized to
+ * fill the HBM, or a framework that keeps all device memory in its own pool -- because a later cudaMalloc there fails or takes
+ * memory the program has promised elsewhere; nor a stepping loop that cannot afford the device-wide synchronisation that
+ * cudaMalloc / cudaFree imply.  Such a caller still has to turn its block levels into the ascending active list of a substep
+ * (T2 of DESIGN.md; level <= ctz(substep)), and this call does exactly that with the same three kernels as
+ * gothic_set_timesteps(acc_pot = NULL), bit for bit the same output, without a context: it calls no cudaMalloc, cudaFree or
+ * any library routine that allocates.
+ *
+ * Where the scratch lives.  The per-tile counts of the ordered compaction (one uint32 per 2048 particles) sit in a file-scope
+ * `static __device__` array of GOTHIC_STATIC_ACTIVE_MAX_N / 2048 words = 128 KiB inside the library image; every GPU that loads
+ * libgothic_b200.so holds those 128 KiB until the process exits, whether or not this call is ever made.
+ *   level         uint8[n] device, in: block level of every particle.
+ *   n             1 .. GOTHIC_STATIC_ACTIVE_MAX_N; a larger n returns GOTHIC_ERR_TOO_LARGE and launches nothing.
+ *   substep       1-based substep of the cycle (> 0).
+ *   active        uint32[n] device, out: ascending indices i with level[i] <= ctz(substep); entries past the count are untouched.
+ *   n_active_dev  uint32 device, out: the count.
+ * Errors: GOTHIC_ERR_ARG (NULL pointer, n = 0, substep = 0, device ordinal above 63), GOTHIC_ERR_TOO_LARGE, GOTHIC_ERR_CUDA
+ * (no device, or a launch failed; cudaGetLastError has the reason).  Asynchronous on `stream` of the CURRENT device.
+ *
+ * First call on a device.  The first call made with a given device current looks up that device's address of the array
+ * (cudaGetSymbolAddress, which may also make the runtime load the library's kernels there) and remembers it; make that call
+ * before the stream is put into capture.  Later calls on that device do no set-up.
+ *
+ * Sharing.  All calls on one device use the same array, and it keeps what the last call left in it.  Nothing in it has to start
+ * at zero (the count pass of a call writes every word that the call's scan then reads), so no clearing is done.  Two calls whose
+ * kernels can overlap on the GPU -- different streams without an ordering between them, or two host threads -- race on the
+ * array and produce garbage: serialise them (same stream, or an event). */
+#define GOTHIC_STATIC_ACTIVE_MAX_N (1u << 26)
+int gothic_active_list_static(const uint8_t *level, uint32_t n, uint32_t substep, uint32_t *active, uint32_t *n_active_dev,
+                              void *stream);
 
 /* Number of kernels this library has launched through this context (bench.py "gpu_launches"). */
 unsigned long long gothic_launch_count(gothic_ctx *ctx);

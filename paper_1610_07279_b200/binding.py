@@ -21,8 +21,9 @@ EXPORTS = [
     "gothic_create", "gothic_destroy", "gothic_strerror", "gothic_last_cuda_error", "gothic_build_tree",
     "gothic_update_moments", "gothic_walk_tree", "gothic_set_timesteps", "gothic_get_tree_view", "gothic_check",
     "gothic_gravity_host", "gothic_block_cycle_host", "gothic_launch_count", "gothic_predict", "gothic_correct", "gothic_set_ball",
-    "gothic_live_init", "gothic_live_step", "gothic_live_get",
+    "gothic_live_init", "gothic_live_step", "gothic_live_get", "gothic_active_list_static",
 ]
+STATIC_ACTIVE_MAX_N = 1 << 26     # GOTHIC_STATIC_ACTIVE_MAX_N of include/gothic.h
 
 
 class GothicError(RuntimeError):
@@ -93,6 +94,8 @@ def load_library():
     L.gothic_live_step.argtypes = [vp, f32, f32, i32, vp, vp]
     L.gothic_live_get.restype = i32
     L.gothic_live_get.argtypes = [vp, C.POINTER(LiveStateStruct)]
+    L.gothic_active_list_static.restype = i32
+    L.gothic_active_list_static.argtypes = [vp, u32, u32, vp, vp, vp]
     L.gothic_launch_count.restype = C.c_ulonglong
     L.gothic_launch_count.argtypes = [vp]
     _lib = L
@@ -111,6 +114,21 @@ def _ptr(t, dtype=None):
 
 def _stream():
     return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def active_list_static(level: torch.Tensor, substep: int, active: torch.Tensor, n_active_dev: torch.Tensor, n: int | None = None):
+    """gothic_active_list_static: the ascending active list of `substep` from the block levels, with no context and no device
+    allocation inside the library.  For hosts that cannot cudaMalloc while they run (device memory already committed to their own
+    arrays or pool, or no room for cudaMalloc's device-wide synchronisation in the step loop): the scratch is a fixed 128 KiB array in
+    the library image, so n <= STATIC_ACTIVE_MAX_N, and calls that may overlap on the GPU must be ordered by the caller.  The
+    tensors are the caller's; `n` defaults to len(level) (pass it to exercise the size check without a 2^26 tensor)."""
+    L = load_library()
+    if not torch.cuda.is_available():
+        raise GothicError("no CUDA device: the GOTHIC hot path has no CPU fallback")
+    rc = L.gothic_active_list_static(_ptr(level, torch.uint8), int(level.shape[0] if n is None else n), int(substep),
+                                     _ptr(active, torch.int32), _ptr(n_active_dev, torch.int32), _stream())
+    if rc != 0:
+        raise GothicError(f"gothic error {rc}: {L.gothic_strerror(rc).decode()}")
 
 
 class _DevView:

@@ -68,6 +68,7 @@ const char *gothic_strerror(int code)
     case GOTHIC_ERR_CAPACITY: return "node pool or traversal stack capacity exceeded";
     case GOTHIC_ERR_CUDA: return "CUDA runtime error";
     case GOTHIC_ERR_UNIMPLEMENTED: return "not implemented";
+    case GOTHIC_ERR_TOO_LARGE: return "n exceeds GOTHIC_STATIC_ACTIVE_MAX_N (the fixed scratch of gothic_active_list_static)";
     default: return "unknown error";
     }
 }

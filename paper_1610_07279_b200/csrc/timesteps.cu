@@ -176,3 +176,52 @@ int gothic_stage_timesteps(gothic_ctx *c, const float4 *acc_pot, uint32_t n, flo
     }
     return GOTHIC_OK;
 }
+
+// ---- gothic_active_list_static: T2 without a context and without any allocation (include/gothic.h) ------------------------
+// For hosts that cannot call cudaMalloc once they are running (all device memory already in their own arrays or pool, or a step
+// loop that must not take cudaMalloc's device-wide synchronisation).  The only scratch T2 needs, the per-tile counts, lives in
+// the library image instead of a gothic_ctx: 32768 words = 128 KiB per GPU that loads the library, for as long as the process
+// lives.  The kernels are the three of gothic_stage_timesteps above, unchanged.
+#include <mutex>
+
+static_assert(GOTHIC_STATIC_ACTIVE_MAX_N % TILE == 0, "whole tiles");
+static __device__ __align__(256) uint32_t g_static_tile_cnt[GOTHIC_STATIC_ACTIVE_MAX_N / TILE];
+
+namespace {
+constexpr int STATIC_MAX_DEVICES = 64;
+std::mutex g_static_mutex;
+// Device address of g_static_tile_cnt on each device, filled by the first call made with that device current.  In host code the
+// name g_static_tile_cnt is only a handle for the runtime, never a pointer a kernel may be given.
+uint32_t *g_static_tile_cnt_addr[STATIC_MAX_DEVICES];
+}
+
+extern "C" int gothic_active_list_static(const uint8_t *level, uint32_t n, uint32_t substep, uint32_t *active,
+                                         uint32_t *n_active_dev, void *stream)
+{
+    if (!level || !active || !n_active_dev || n == 0 || substep == 0) return GOTHIC_ERR_ARG;
+    if (n > GOTHIC_STATIC_ACTIVE_MAX_N) return GOTHIC_ERR_TOO_LARGE;
+    int device = -1;
+    if (cudaGetDevice(&device) != cudaSuccess) return GOTHIC_ERR_CUDA;
+    if (device < 0 || device >= STATIC_MAX_DEVICES) return GOTHIC_ERR_ARG;
+    uint32_t *tile_cnt;
+    {
+        std::lock_guard<std::mutex> lock(g_static_mutex);
+        tile_cnt = g_static_tile_cnt_addr[device];
+        if (!tile_cnt) {                       // set-up, once per device, with that device current
+            void *p = nullptr;
+            if (cudaGetSymbolAddress(&p, g_static_tile_cnt) != cudaSuccess || !p) return GOTHIC_ERR_CUDA;
+            tile_cnt = g_static_tile_cnt_addr[device] = static_cast<uint32_t *>(p);
+        }
+    }
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    const int ctz = __builtin_ctz(substep);
+    const uint32_t ntiles = (n + TILE - 1) / TILE;
+    // no word of tile_cnt needs to be zero on entry: k_active_count stores (not adds) one count per tile, the scan reads only those
+    k_active_count<<<ntiles, TPB, 0, s>>>(level, n, ctz, tile_cnt);
+    if (cudaGetLastError() != cudaSuccess) return GOTHIC_ERR_CUDA;
+    k_active_scan<<<1, 1024, 0, s>>>(tile_cnt, ntiles, n_active_dev);
+    if (cudaGetLastError() != cudaSuccess) return GOTHIC_ERR_CUDA;
+    k_active_scatter<<<ntiles, TPB, 0, s>>>(level, n, ctz, tile_cnt, active);
+    if (cudaGetLastError() != cudaSuccess) return GOTHIC_ERR_CUDA;
+    return GOTHIC_OK;
+}
