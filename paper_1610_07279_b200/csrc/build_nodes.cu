@@ -176,7 +176,7 @@ __global__ void __launch_bounds__(TPB) k_emit_nodes(const uint32_t *__restrict__
                                                      uint32_t *__restrict__ node_last)
 {
     __shared__ uint32_t wcnt[2][GOTHIC_NLEVP1][NROW];   // counts per (row, warp) in key order -> exclusive prefix + tile base + level offset
-    if (flags[0]) return;
+    if (flags[0] | flags[3]) return;      // pool overflow, or keys the fast sort left unordered (end counts may then exceed start counts: ids past n_nodes)
     for (int t = threadIdx.x; t < 2 * GOTHIC_NLEVP1 * NROW; t += TPB) (&wcnt[0][0][0])[t] = 0u;
     const uint32_t base = blockIdx.x * (uint32_t)TILE;
     const int warp = threadIdx.x >> 5;
