@@ -226,8 +226,26 @@ __global__ void __launch_bounds__(SORT_TPB, GOTHIC_SORT_CTAS) k_sort_onesweep(co
     }
 }
 
+// Is the run of equal upper bits that holds entry i longer than FIX_LONG_MAX?  Two probes half that far away answer "no" for almost every
+// caller (a run of more than 2 H entries reaches at least H to one side of each of its members); only then are the run's ends found by
+// bisection on the upper bits, which the fast passes have fully sorted.  Reads upper bits only: k_sort_fix_short never changes those.
+__device__ __forceinline__ bool run_too_long(const uint64_t *__restrict__ key, uint32_t n, uint32_t i, uint64_t top)
+{
+    constexpr uint32_t H = FIX_LONG_MAX / 2;
+    const bool far = (i >= H && (key[i - H] >> LOW_BITS) == top) || (i + H < n && (key[i + H] >> LOW_BITS) == top);
+    if (!far) return false;
+    uint32_t lo = 0, hi = i;                       // first entry of the run: smallest j with top(j) == top
+    while (lo < hi) { const uint32_t mid = lo + (hi - lo) / 2; if ((key[mid] >> LOW_BITS) < top) lo = mid + 1; else hi = mid; }
+    const uint32_t first = lo;
+    lo = i + 1; hi = n;                            // one past its last entry
+    while (lo < hi) { const uint32_t mid = lo + (hi - lo) / 2; if ((key[mid] >> LOW_BITS) <= top) lo = mid + 1; else hi = mid; }
+    return lo - first > (uint32_t)FIX_LONG_MAX;
+}
+
 // Runs of equal upper bits (key >> LOW_BITS) after the fast passes: inside a run the keys are in ascending original index and
-// still have to be ordered by their low bits, stably.  One thread per run start; runs that are already in order cost one scan.
+// still have to be ordered by their low bits, stably.  One thread per run start measures the run, up to FIX_LONG_MAX + 1 entries and no
+// further; runs that are already in order cost that one scan.  A run too long for the fix-up kernels needs the eight-pass build unless it is
+// in order already (coincident particles): that is decided in parallel, by every entry that sees a larger key right before it in its run.
 __global__ void __launch_bounds__(SORT_TPB) k_sort_fix_short(uint64_t *__restrict__ key, uint32_t *__restrict__ val, uint32_t n,
                                                               uint2 *__restrict__ long_runs, uint32_t long_cap, uint32_t *__restrict__ n_long,
                                                               uint32_t *__restrict__ flags)
@@ -236,18 +254,26 @@ __global__ void __launch_bounds__(SORT_TPB) k_sort_fix_short(uint64_t *__restric
     if (i >= n) return;
     const uint64_t ki = key[i];
     const uint64_t top = ki >> LOW_BITS;
-    if (i > 0 && (key[i - 1] >> LOW_BITS) == top) return;          // not the first of its run
+    if (i > 0) {
+        const uint64_t kp = key[i - 1];
+        if ((kp >> LOW_BITS) == top) {                              // not the first of its run
+            // (a short run may be mid-way through its insertion sort here: kp > ki is then unreliable, but such a run is never too long)
+            if (kp > ki && *reinterpret_cast<volatile uint32_t *>(flags + 3) == 0u && run_too_long(key, n, i, top)) atomicExch(flags + 3, 1u);
+            return;
+        }
+    }
     if (i + 1 >= n || (key[i + 1] >> LOW_BITS) != top) return;      // a run of one
     uint32_t len = 1;
     bool ordered = true;
     uint64_t prev = ki;
-    while (i + len < n) {
+    while (i + len < n && len <= (uint32_t)FIX_LONG_MAX) {
         const uint64_t kj = key[i + len];
         if ((kj >> LOW_BITS) != top) break;
         ordered = ordered && prev <= kj;
         prev = kj;
         len++;
     }
+    if (len > (uint32_t)FIX_LONG_MAX) return;                       // too long to fix here; its inversions, if any, raise flags[3] above
     if (ordered) return;
     if (len <= (uint32_t)FIX_SHORT_MAX) {
         for (uint32_t a = 1; a < len; a++) {                       // stable insertion sort: an entry passes strictly larger keys only
@@ -257,11 +283,11 @@ __global__ void __launch_bounds__(SORT_TPB) k_sort_fix_short(uint64_t *__restric
             while (b > 0 && key[i + b - 1] > k) { key[i + b] = key[i + b - 1]; val[i + b] = val[i + b - 1]; b--; }
             key[i + b] = k; val[i + b] = v;
         }
-    } else if (len <= (uint32_t)FIX_LONG_MAX) {
+    } else {
         const uint32_t at = atomicAdd(n_long, 1u);
         if (at < long_cap) long_runs[at] = make_uint2(i, len);
         else atomicExch(flags + 3, 1u);
-    } else atomicExch(flags + 3, 1u);
+    }
 }
 
 // One CTA per long run: rank of an entry = number of entries with a smaller key, or with an equal key and an earlier place.

@@ -80,6 +80,35 @@ def test_sort_runs_of_equal_upper_bits(oracle, n_clump, spread, kind):
     assert runs.max() >= min(n_clump // 8, 33) or n_clump < 100       # the case really has long runs of equal upper bits
 
 
+def test_sort_long_ordered_run_of_coincident_particles(oracle):
+    """A run of equal upper key bits far longer than the fix-up kernels take, but already in order (50 000 coincident particles: equal keys,
+    ascending original index), next to a too-long run of distinct particles in a second build: the run head stops measuring at the limit and
+    the ordered / unordered decision is taken in parallel by the entries of the run; perm is the oracle's in both."""
+    rng = np.random.default_rng(77)
+    n_far, n_same = 3000, 50000
+    pos = np.zeros((n_far + n_same + 600, 4), np.float32)
+    pos[:n_far, :3] = rng.uniform(-16.0, 16.0, (n_far, 3))
+    pos[n_far:n_far + n_same, :3] = np.asarray((1.25, -2.5, 0.375), np.float32)
+    pos[n_far + n_same:, :3] = np.asarray((5.0, -3.0, 2.0), np.float32) + rng.uniform(-3e-4, 3e-4, (600, 3)).astype(np.float32)
+    pos[:, 3] = 1.0 / pos.shape[0]
+    order = rng.permutation(pos.shape[0])
+    from gpu_util import gpu_build
+
+    def check(p, kind):       # index work only (one leaf of 50 000 particles is outside the moment tolerances of _check_build)
+        g, v = gpu_build(p, key_kind=kind)
+        t = oracle.build_tree(p, key_kind=kind)
+        assert np.array_equal(v["key"], t.key) and np.array_equal(v["perm"], t.perm) and np.array_equal(v["pos_m_sorted"], t.pos_sorted)
+        assert v["n_nodes"] == t.n_nodes and np.array_equal(v["node_head"], t.head) and np.array_equal(v["node_num"], t.num)
+        assert np.array_equal(v["node_child"], t.child) and np.array_equal(v["node_level"], t.level)
+        g.close()
+        top = t.key >> np.uint64(23)
+        return np.diff(np.flatnonzero(np.concatenate([[True], top[1:] != top[:-1], [True]]))).max()
+
+    assert check(pos[order], 0) >= n_same
+    pos[n_far:n_far + n_same, :3] += rng.uniform(-1e-5, 1e-5, (n_same, 3)).astype(np.float32)      # now distinct: the eight-pass repeat
+    assert check(pos[order], 1) > 2048
+
+
 def test_build_degenerate_inputs(oracle):
     # all particles at one point: root cube side 1, one level-21 leaf chain
     pos = np.tile(np.array([[0.25, -1.0, 3.0, 0.01]], np.float32), (100, 1))
