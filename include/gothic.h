@@ -200,14 +200,18 @@ int gothic_correct(gothic_ctx *ctx, const uint32_t *active, uint32_t n_active, c
  *   |a_old| = the particle's last |a|) -> correct the active particles (eq. 17) with level migration (reading R15).
  * When t_now reaches n_substeps = 2^(n_levels-1) every particle is synchronised: the levels are taken afresh from the new
  * accelerations (gothic_set_timesteps' arithmetic), t_now and every t_last return to 0, and one 8-byte read-back of
- * {e_min, n_levels} synchronises the stream (once per cycle).  Everything else is asynchronous.
+ * {e_min, n_levels} synchronises the stream (once per cycle).  A rebuild step synchronises once as well (gothic_build_tree reads back
+ * the node count).  Everything else is asynchronous.
  *
  * gothic_live_init: pos_m float4[n], vel float4[n] (vx, vy, vz, unused) in ORIGINAL order; builds the tree, bootstraps the
  *   accelerations with an opening-angle walk (eq. 2, theta_boot; R7), takes the first levels.  Synchronises.
  * gothic_live_step: rebuild != 0 rebuilds the tree in this step.  n_interactions (device, optional) accumulates P:331's count.
  * gothic_live_get: device pointers of the current state (tree order; orig[s] = original index of row s) and the clock.
  *   The pointers stay valid until the next rebuild step or gothic_live_init; rows change with every step.
- * Errors: GOTHIC_ERR_STATE before gothic_live_init; GOTHIC_ERR_ARG for bad arguments. */
+ * Errors: GOTHIC_ERR_ARG for bad arguments; GOTHIC_ERR_STATE before a successful gothic_live_init, after any other build on this
+ *   context (gothic_build_tree, gothic_gravity_host, gothic_block_cycle_host: the rows no longer belong to the tree, even for the same
+ *   n), and after a gothic_live_step that failed (its rows may be half-way through the step; the clock t_now and `steps` advance only
+ *   when every stage of a step has been launched): call gothic_live_init again. */
 typedef struct gothic_live_state {
     uint32_t n;
     uint32_t t_now;               /* substep index within the cycle, 0 .. n_substeps */

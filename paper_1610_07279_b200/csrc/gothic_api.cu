@@ -181,6 +181,7 @@ int gothic_build_tree(gothic_ctx *c, const float *pos_m, uint32_t n, int key_kin
     if (rc != GOTHIC_OK) return rc == GOTHIC_RETRY_FULL_SORT ? GOTHIC_ERR_STATE : rc;
     if ((rc = gothic_stage_moments(c, s)) != GOTHIC_OK) return rc;
     c->built = true;
+    c->tree_gen++;
     return GOTHIC_OK;
 }
 

@@ -28,12 +28,14 @@ struct gothic_ctx {
     int n_leaf;
     int device;
     int num_sms;
+    int radius_blocks_per_sm;   // resident CTAs of k_node_radius per SM, asked of the runtime once (0 = not yet)
     // state of the last build
     uint32_t n;
     uint32_t n_nodes;
     uint32_t n_levels_tree;
     uint32_t h_level_ofs[GOTHIC_NLEVP1 + 1];
     bool built;
+    unsigned long long tree_gen;   // number of successful gothic_build_tree calls: lets gothic_live_step see a build that was not its own
     unsigned long long launches;
     cudaError_t last_err;
     // device buffers

@@ -109,6 +109,8 @@ struct gothic_live {
     int e_min, n_levels;
     int key_kind, n_leaf, max_levels;
     float eps, eta;
+    bool ready;                               // set at the end of gothic_live_init, cleared by any stage that fails: the rows may then be half-way through a step
+    unsigned long long tree_gen;              // c->tree_gen after the live run's own last build
 };
 
 void gothic_live_free(gothic_ctx *c)
@@ -150,6 +152,48 @@ int live_new_cycle(gothic_ctx *c, gothic_live *L, cudaStream_t s)
     L->n_levels = h[1];
     L->n_sub = 1u << (h[1] - 1);
     L->t_now = 0;
+    return GOTHIC_OK;
+}
+
+// the stages of one block step; the clock and the step count are committed only after the last launch has been accepted
+int live_step_stages(gothic_ctx *c, gothic_live *L, float delta_acc, float r_crit, int rebuild, unsigned long long *n_interactions, void *stream)
+{
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    const uint32_t n = L->n, grid = (n + TPB - 1) / TPB;
+    const float dt_unit = ldexpf(1.0f, L->e_min);
+    int rc;
+    const uint32_t t_next = L->t_now + 1u;
+    int k = L->cur;
+    if (rebuild) {
+        // predicted positions in the old order -> new tree (whose gathered copy is the prediction in the new order) -> rows re-ordered
+        k_predict<<<grid, TPB, 0, s>>>(L->pos[k], L->vel[k], L->acc[k], L->t_last[k], t_next, dt_unit, n, L->pred);
+        GOTHIC_LAUNCH_OK(c);
+        if ((rc = gothic_build_tree(c, reinterpret_cast<const float *>(L->pred), n, L->key_kind, L->n_leaf, stream)) != GOTHIC_OK) return rc;
+        L->tree_gen = c->tree_gen;
+        k_permute_state<<<grid, TPB, 0, s>>>(c->idx[c->cur], n, L->pos[k], L->vel[k], L->acc[k], L->amag[k], L->t_last[k], L->level[k], L->orig[k],
+                                              L->pos[k ^ 1], L->vel[k ^ 1], L->acc[k ^ 1], L->amag[k ^ 1], L->t_last[k ^ 1], L->level[k ^ 1], L->orig[k ^ 1]);
+        GOTHIC_LAUNCH_OK(c);
+        k = L->cur = k ^ 1;
+        L->steps_since_rebuild = 0;
+    } else {
+        // the prediction goes straight into the tree's particle array; links stay, moments are recomputed (PAPER.md:62)
+        k_predict<<<grid, TPB, 0, s>>>(L->pos[k], L->vel[k], L->acc[k], L->t_last[k], t_next, dt_unit, n, c->pos_sorted);
+        GOTHIC_LAUNCH_OK(c);
+        if ((rc = gothic_stage_moments(c, s)) != GOTHIC_OK) return rc;
+        L->steps_since_rebuild += 1u;
+    }
+    const float cconst = timestep_constant(L->eps, L->eta);
+    if ((rc = gothic_stage_timesteps(c, nullptr, n, cconst, L->max_levels, t_next, L->level[k], L->active, L->n_active, nullptr, s)) != GOTHIC_OK) return rc;
+    if ((rc = gothic_stage_walk(c, L->active, 0, L->n_active, L->eps, GOTHIC_MAC_ACCELERATION, delta_acc, r_crit, L->amag[k], L->acc_new, L->amag[k],
+                                n_interactions, s)) != GOTHIC_OK) return rc;
+    int cgrid = (int)grid;
+    if (cgrid > c->num_sms * 16) cgrid = c->num_sms * 16;
+    k_correct<<<cgrid, TPB, 0, s>>>(L->active, 0, L->n_active, c->pos_sorted, L->acc_new, t_next, dt_unit, L->pos[k], L->vel[k], L->acc[k], L->t_last[k],
+                                    L->level[k], cconst, L->e_min, L->max_levels);
+    GOTHIC_LAUNCH_OK(c);
+    L->t_now = t_next;
+    L->steps += 1ull;
+    if (t_next == L->n_sub) return live_new_cycle(c, L, s);      // everybody synchronised: fresh levels, clock back to zero
     return GOTHIC_OK;
 }
 
@@ -227,49 +271,22 @@ int gothic_live_init(gothic_ctx *c, const float *pos_m, const float *vel, uint32
     L->steps = 0;
     L->steps_since_rebuild = 0;
     if ((rc = live_new_cycle(c, L, s)) != GOTHIC_OK) return rc;
-    return gothic_check(c, stream);
+    if ((rc = gothic_check(c, stream)) != GOTHIC_OK) return rc;
+    L->tree_gen = c->tree_gen;
+    L->ready = true;
+    return GOTHIC_OK;
 }
 
 int gothic_live_step(gothic_ctx *c, float delta_acc, float r_crit, int rebuild, unsigned long long *n_interactions, void *stream)
 {
     if (!c || !(delta_acc >= 0.0f) || !(r_crit >= 0.0f)) return GOTHIC_ERR_ARG;
     gothic_live *L = c->live;
-    if (!L || !c->built || c->n != L->n) return GOTHIC_ERR_STATE;     // (a gothic_build_tree of another particle set in between ends the live run)
-    cudaStream_t s = static_cast<cudaStream_t>(stream);
-    const uint32_t n = L->n, grid = (n + TPB - 1) / TPB;
-    const float dt_unit = ldexpf(1.0f, L->e_min);
-    int rc;
-    L->t_now += 1u;
-    int k = L->cur;
-    if (rebuild) {
-        // predicted positions in the old order -> new tree (whose gathered copy is the prediction in the new order) -> rows re-ordered
-        k_predict<<<grid, TPB, 0, s>>>(L->pos[k], L->vel[k], L->acc[k], L->t_last[k], L->t_now, dt_unit, n, L->pred);
-        GOTHIC_LAUNCH_OK(c);
-        if ((rc = gothic_build_tree(c, reinterpret_cast<const float *>(L->pred), n, L->key_kind, L->n_leaf, stream)) != GOTHIC_OK) return rc;
-        k_permute_state<<<grid, TPB, 0, s>>>(c->idx[c->cur], n, L->pos[k], L->vel[k], L->acc[k], L->amag[k], L->t_last[k], L->level[k], L->orig[k],
-                                              L->pos[k ^ 1], L->vel[k ^ 1], L->acc[k ^ 1], L->amag[k ^ 1], L->t_last[k ^ 1], L->level[k ^ 1], L->orig[k ^ 1]);
-        GOTHIC_LAUNCH_OK(c);
-        k = L->cur = k ^ 1;
-        L->steps_since_rebuild = 0;
-    } else {
-        // the prediction goes straight into the tree's particle array; links stay, moments are recomputed (PAPER.md:62)
-        k_predict<<<grid, TPB, 0, s>>>(L->pos[k], L->vel[k], L->acc[k], L->t_last[k], L->t_now, dt_unit, n, c->pos_sorted);
-        GOTHIC_LAUNCH_OK(c);
-        if ((rc = gothic_stage_moments(c, s)) != GOTHIC_OK) return rc;
-        L->steps_since_rebuild += 1u;
-    }
-    const float cconst = timestep_constant(L->eps, L->eta);
-    if ((rc = gothic_stage_timesteps(c, nullptr, n, cconst, L->max_levels, L->t_now, L->level[k], L->active, L->n_active, nullptr, s)) != GOTHIC_OK) return rc;
-    if ((rc = gothic_stage_walk(c, L->active, 0, L->n_active, L->eps, GOTHIC_MAC_ACCELERATION, delta_acc, r_crit, L->amag[k], L->acc_new, L->amag[k],
-                                n_interactions, s)) != GOTHIC_OK) return rc;
-    int cgrid = (int)grid;
-    if (cgrid > c->num_sms * 16) cgrid = c->num_sms * 16;
-    k_correct<<<cgrid, TPB, 0, s>>>(L->active, 0, L->n_active, c->pos_sorted, L->acc_new, L->t_now, dt_unit, L->pos[k], L->vel[k], L->acc[k], L->t_last[k],
-                                    L->level[k], cconst, L->e_min, L->max_levels);
-    GOTHIC_LAUNCH_OK(c);
-    L->steps += 1ull;
-    if (L->t_now == L->n_sub) return live_new_cycle(c, L, s);      // everybody synchronised: fresh levels, clock back to zero
-    return GOTHIC_OK;
+    // not after a failed gothic_live_init / gothic_live_step, and not after somebody else's build on this context (gothic_build_tree,
+    // gothic_gravity_host, gothic_block_cycle_host): the rows would no longer belong to the tree, even with the same n
+    if (!L || !L->ready || !c->built || c->n != L->n || c->tree_gen != L->tree_gen) return GOTHIC_ERR_STATE;
+    const int rc = live_step_stages(c, L, delta_acc, r_crit, rebuild, n_interactions, stream);
+    if (rc != GOTHIC_OK) L->ready = false;       // gothic_live_init starts over
+    return rc;
 }
 
 int gothic_live_get(gothic_ctx *c, gothic_live_state *out)

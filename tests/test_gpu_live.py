@@ -28,7 +28,9 @@ def _state(g):
     return out
 
 
-@pytest.mark.parametrize("model,n,every", [("plummer", 6000, 3), ("hernquist", 9001, 1), ("nfw", 8192, 1000)])
+# the 2^20 case runs one cycle: the rebuild from predicted positions (nearly sorted input, k_permute_state) at a size where the sort's
+# fix-up kernels and full 2048-key event tiles see moved particles
+@pytest.mark.parametrize("model,n,every", [("plummer", 6000, 3), ("hernquist", 9001, 1), ("nfw", 8192, 1000), ("nfw", 1 << 20, 2)])
 def test_live_steps_stagewise_vs_oracle(oracle, model, n, every):
     from gpu_util import dev, view_to_numpy
     from paper_1610_07279_b200.binding import Gothic
@@ -49,7 +51,7 @@ def test_live_steps_stagewise_vs_oracle(oracle, model, n, every):
     cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
     seen_migration = False
     steps = 0
-    for cycle in range(2):
+    for cycle in range(2 if n < (1 << 18) else 1):
         for _ in range(st["n_substeps"]):
             prev, t, unit = st, st["t_now"] + 1, 2.0 ** st["e_min"]
             rebuild = steps % every == every - 1
@@ -96,6 +98,34 @@ def test_live_steps_stagewise_vs_oracle(oracle, model, n, every):
             for k in rows:
                 assert np.array_equal(st[k], rows[k]), (k, steps)
     assert seen_migration and steps >= 4
+    g.close()
+
+
+def test_live_step_refuses_a_tree_that_is_not_its_own():
+    """Another build on the same context between two live steps -- same n, other particles -- ends the live run: the rows no longer belong
+    to the tree.  The step returns GOTHIC_ERR_STATE and leaves the clock where it was; gothic_live_init starts a new run."""
+    from gpu_util import dev
+    from paper_1610_07279_b200.binding import Gothic, GothicError
+    n, eps = 4000, 1.0 / 64
+    pos = W.plummer(n, seed=21)
+    vel = W.isotropic_velocities(pos, "plummer", seed=22)
+    g = Gothic(n)
+    with pytest.raises(GothicError, match="-2"):
+        g.live_step(delta_acc=2.0 ** -8)                     # before gothic_live_init
+    g.live_init(dev(pos), dev(vel), eps=eps, eta=0.25, max_levels=4, theta_boot=0.5)
+    g.live_step(delta_acc=2.0 ** -8, r_crit=0.5, rebuild=True)       # the run's own rebuild is fine
+    g.live_step(delta_acc=2.0 ** -8, r_crit=0.5)
+    before = g.live_get(arrays=False)
+    assert before["steps"] == 2
+    g.build_tree(dev(W.plummer(n, seed=23)))                 # somebody else's tree, same n
+    with pytest.raises(GothicError, match="-2"):
+        g.live_step(delta_acc=2.0 ** -8, r_crit=0.5)
+    after = g.live_get(arrays=False)
+    assert (after["t_now"], after["steps"]) == (before["t_now"], before["steps"])
+    g.live_init(dev(pos), dev(vel), eps=eps, eta=0.25, max_levels=4, theta_boot=0.5)
+    g.live_step(delta_acc=2.0 ** -8, r_crit=0.5)
+    g.check()
+    assert g.live_get(arrays=False)["steps"] == 1
     g.close()
 
 
