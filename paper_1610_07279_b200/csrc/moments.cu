@@ -69,14 +69,12 @@ __global__ void __launch_bounds__(TPB) k_leaf_moments(uint32_t n_nodes, const fl
     node_B2[J] = B2;
 }
 
-__global__ void __launch_bounds__(TPB) k_internal_moments(uint32_t first, uint32_t count, const uint32_t *__restrict__ node_child,
-                                                           const uint8_t *__restrict__ node_nchild, float4 *__restrict__ node_msum,
-                                                           float4 *__restrict__ node_com, uint32_t *__restrict__ node_b2bits,
-                                                           const uint32_t *__restrict__ node_parent, float4 *__restrict__ node_up, float *__restrict__ node_B2)
+// m_J, r_J (and B_2) of one internal node from its children, which the level below has finished
+__device__ __forceinline__ void internal_moment_of(uint32_t J, const uint32_t *__restrict__ node_child, const uint8_t *__restrict__ node_nchild,
+                                                   float4 *node_msum, float4 *node_com, uint32_t *node_b2bits,
+                                                   const uint32_t *__restrict__ node_parent, float4 *node_up, float *node_B2)
 {
-    const uint32_t t = blockIdx.x * TPB + threadIdx.x;
-    if (t >= count) return;
-    const uint32_t J = first + t, c = node_child[J];
+    const uint32_t c = node_child[J];
     if (c == GOTHIC_LEAF) return;
     const uint32_t nc = node_nchild[J];
     float4 ms = node_msum[c];
@@ -94,6 +92,34 @@ __global__ void __launch_bounds__(TPB) k_internal_moments(uint32_t first, uint32
         B2 += fmaf(q.w, fmaf(dz, dz, fmaf(dy, dy, dx * dx)), node_B2[c + k]);
     }
     node_B2[J] = B2;
+}
+
+__global__ void __launch_bounds__(TPB) k_internal_moments(uint32_t first, uint32_t count, const uint32_t *__restrict__ node_child,
+                                                           const uint8_t *__restrict__ node_nchild, float4 *node_msum,
+                                                           float4 *node_com, uint32_t *node_b2bits,
+                                                           const uint32_t *__restrict__ node_parent, float4 *node_up, float *node_B2)
+{
+    const uint32_t t = blockIdx.x * TPB + threadIdx.x;
+    if (t >= count) return;
+    internal_moment_of(first + t, node_child, node_nchild, node_msum, node_com, node_b2bits, node_parent, node_up, node_B2);
+}
+
+// A run of consecutive SMALL levels (the top of the tree, and its sparse deepest levels) in one launch: one CTA sweeps level l_from, then
+// l_from - 1, ... down to l_to, a block barrier between levels (the children of a level were written by this CTA one barrier earlier).
+// Same per-node arithmetic as k_internal_moments, so the moments do not change by a bit; it only saves the launches.
+constexpr int SMALL_TPB = 1024;
+constexpr uint32_t SMALL_LEVEL_MAX = 8192;      // nodes: at most 8 per thread and level
+__global__ void __launch_bounds__(SMALL_TPB) k_internal_moments_small(const uint32_t *__restrict__ level_ofs, int l_from, int l_to,
+                                                                       const uint32_t *__restrict__ node_child, const uint8_t *__restrict__ node_nchild,
+                                                                       float4 *node_msum, float4 *node_com, uint32_t *node_b2bits,
+                                                                       const uint32_t *__restrict__ node_parent, float4 *node_up, float *node_B2)
+{
+    for (int L = l_from; L >= l_to; L--) {
+        const uint32_t first = level_ofs[L], count = level_ofs[L + 1] - first;
+        for (uint32_t t = threadIdx.x; t < count; t += SMALL_TPB)
+            internal_moment_of(first + t, node_child, node_nchild, node_msum, node_com, node_b2bits, node_parent, node_up, node_B2);
+        __syncthreads();
+    }
 }
 
 // Persistent warps, each sweeping a contiguous range of sorted particles 32 at a time.  Lane L of a warp remembers the
@@ -249,16 +275,29 @@ int gothic_stage_moments(gothic_ctx *c, cudaStream_t s)
     const uint32_t grid = (m + TPB - 1) / TPB;
     k_leaf_moments<<<grid, TPB, 0, s>>>(m, c->pos_sorted, c->node_head, c->node_num, c->node_child, c->node_msum, c->node_com, c->node_b2bits, c->node_parent, c->node_up, c->b2_enabled ? c->node_B2 : nullptr);
     GOTHIC_LAUNCH_OK(c);
-    for (int L = (int)c->n_levels_tree - 2; L >= 0; L--) {
+    for (int L = (int)c->n_levels_tree - 2; L >= 0;) {
         const uint32_t first = c->h_level_ofs[L], count = c->h_level_ofs[L + 1] - first;
-        if (!count) continue;
+        if (!count) { L--; continue; }
+        if (count <= SMALL_LEVEL_MAX) {           // this level and the small ones right above it: one CTA, one launch
+            int l_to = L;
+            while (l_to > 0 && c->h_level_ofs[l_to] - c->h_level_ofs[l_to - 1] <= SMALL_LEVEL_MAX) l_to--;
+            k_internal_moments_small<<<1, SMALL_TPB, 0, s>>>(c->level_ofs, L, l_to, c->node_child, c->node_nchild, c->node_msum, c->node_com, c->node_b2bits,
+                                                             c->node_parent, c->node_up, c->b2_enabled ? c->node_B2 : nullptr);
+            GOTHIC_LAUNCH_OK(c);
+            L = l_to - 1;
+            continue;
+        }
         k_internal_moments<<<(count + TPB - 1) / TPB, TPB, 0, s>>>(first, count, c->node_child, c->node_nchild, c->node_msum, c->node_com, c->node_b2bits, c->node_parent, c->node_up, c->b2_enabled ? c->node_B2 : nullptr);
         GOTHIC_LAUNCH_OK(c);
+        L--;
     }
     {
-        int per_sm = 0;
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_node_radius, TPB, 0);
-        if (per_sm < 1) per_sm = 1;
+        if (c->radius_blocks_per_sm < 1) {
+            int q = 0;
+            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&q, k_node_radius, TPB, 0) != cudaSuccess || q < 1) q = 1;
+            c->radius_blocks_per_sm = q;
+        }
+        const int per_sm = c->radius_blocks_per_sm;
         const uint32_t blocks = (uint32_t)(c->num_sms * per_sm), warps = blocks * (TPB / 32);     // one resident wave
         const uint32_t per_warp = (((c->n + warps - 1) / warps + 31u) / 32u) * 32u;
         k_node_radius<<<blocks, TPB, 0, s>>>(c->n, per_warp, c->pos_sorted, c->leaf_of, c->leaf_level, c->node_head, c->node_num, c->node_up, c->node_b2bits);
