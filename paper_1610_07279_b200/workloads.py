@@ -14,7 +14,7 @@ from __future__ import annotations
 import numpy as np
 
 __all__ = [
-    "plummer", "hernquist", "nfw", "m31_like", "make_config", "CONFIGS", "random_active_subset", "isotropic_velocities", "LIVE_CONFIGS", "make_live_config",
+    "plummer", "hernquist", "nfw", "m31_like", "make_config", "CONFIGS", "random_active_subset", "isotropic_velocities", "LIVE_CONFIGS", "make_live_config", "m31_velocities",
 ]
 
 
@@ -128,7 +128,7 @@ def nfw(n: int, seed: int = 1, rs: float = 1.0, rmax: float = 10.0) -> np.ndarra
     return _finish(rng, _isotropic(rng, _r_nfw(rng, n, rs, rmax)))
 
 
-def m31_like(n: int, seed: int = 1) -> np.ndarray:
+def m31_like(n: int, seed: int = 1, components: bool = False):
     """NFW halo 81 % + Hernquist bulge 8 % + exponential disk 11 % by mass (BASELINE.json configs[3]);
     equal-mass particles, so the split is by count.  Scale radii in units of R_d = 1:
     halo r_s = 1.413 (cut at 10 r_s), bulge a = 0.113 (cut at 100 a), disk R_d = 1, z_d = 0.1."""
@@ -140,8 +140,49 @@ def m31_like(n: int, seed: int = 1) -> np.ndarray:
     bulge = _isotropic(rng, _r_hernquist(rng, n_bulge, 0.113, 11.3))
     disk = _disk(rng, n_disk, 1.0, 0.1, 10.0)
     xyz = np.concatenate([halo, bulge, disk], axis=0)
-    xyz = xyz[rng.permutation(n)]
-    return _finish(rng, xyz)
+    perm = rng.permutation(n)
+    xyz = xyz[perm]
+    pos_m = _finish(rng, xyz)
+    if not components:
+        return pos_m
+    comp = np.concatenate([np.zeros(n_halo, np.uint8), np.ones(n_bulge, np.uint8), np.full(n_disk, 2, np.uint8)])[perm]
+    return pos_m, comp      # component of every particle: 0 halo, 1 bulge, 2 disk (for m31_velocities)
+
+
+def m31_velocities(pos_m: np.ndarray, comp: np.ndarray, seed: int = 2) -> np.ndarray:
+    """Velocities (vx, vy, vz, 0) float32 for a live run of m31_like: a STAND-IN for the paper's M31 initial conditions (which come from a
+    distribution-function code), good enough for orbits, level migration and tree ageing, not an equilibrium model.
+    Everything is taken from the particles themselves under a spherical average (G = 1): M(<r) by sorting the radii, rho(r) from counts in
+    256 logarithmic shells.  Halo and bulge particles: isotropic Gaussian with the spherical Jeans dispersion of the total profile,
+    sigma^2(r) = (1/rho) int_r^inf rho M / s^2 ds.  Disk particles: the circular speed sqrt(M(<r)/r) about the z axis plus an isotropic
+    Gaussian of 15 % of it (in place of the epicyclic dispersions)."""
+    n = pos_m.shape[0]
+    xyz = pos_m[:, :3].astype(np.float64)
+    r = np.maximum(np.linalg.norm(xyz, axis=1), 1e-9)
+    order = np.argsort(r, kind="stable")
+    m_enc = np.empty(n)
+    m_enc[order] = np.cumsum(pos_m[order, 3].astype(np.float64))
+    edges = np.geomspace(max(r.min(), 1e-6), r.max() * (1 + 1e-9), 257)
+    mass_in, _ = np.histogram(r, bins=edges, weights=pos_m[:, 3].astype(np.float64))
+    mid = np.sqrt(edges[1:] * edges[:-1])
+    rho = mass_in / (4.0 / 3.0 * np.pi * (edges[1:] ** 3 - edges[:-1] ** 3))
+    m_mid = np.interp(mid, r[order], m_enc[order])
+    f = rho * m_mid / mid ** 2
+    seg = 0.5 * (f[1:] + f[:-1]) * np.diff(mid)
+    tail = np.concatenate([np.cumsum(seg[::-1])[::-1], [0.0]])
+    full = mass_in > 0                                                    # empty shells (far inside, far outside) take their neighbours' value
+    sig = np.sqrt(np.interp(r, mid[full], tail[full] / rho[full]))
+    rng = _rng(seed)
+    vel = np.zeros((n, 4), np.float32)
+    v = rng.normal(size=(n, 3)) * sig[:, None]
+    disk = comp == 2
+    vc = np.sqrt(m_enc[disk] / r[disk])
+    R = np.maximum(np.hypot(xyz[disk, 0], xyz[disk, 1]), 1e-9)
+    v[disk] = rng.normal(size=(int(disk.sum()), 3)) * (0.15 * vc)[:, None]
+    v[disk, 0] += -vc * xyz[disk, 1] / R
+    v[disk, 1] += vc * xyz[disk, 0] / R
+    vel[:, :3] = v.astype(np.float32)
+    return vel
 
 
 def isotropic_velocities(pos_m: np.ndarray, model: str, seed: int = 2) -> np.ndarray:
@@ -201,6 +242,8 @@ LIVE_CONFIGS = {
     "plummer_2p20_live": dict(model="plummer", n=1 << 20, eps=2.0 ** -7, delta_acc=2.0 ** -9, r_crit=1.0, group_size=32),
     "nfw_2p22_live": dict(model="nfw", n=1 << 22, eps=2.0 ** -8, delta_acc=2.0 ** -9, r_crit=0.5, group_size=32),
     "nfw_2p24_live": dict(model="nfw", n=1 << 24, eps=2.0 ** -8, delta_acc=2.0 ** -9, r_crit=0.5, group_size=32),
+    # the paper's headline model under live stepping; velocities are m31_velocities' stand-in
+    "m31_2p24_live": dict(model="m31_like", n=1 << 24, eps=2.0 ** -8, delta_acc=2.0 ** -9, r_crit=0.5, group_size=32),
 }
 
 
@@ -209,8 +252,12 @@ def make_live_config(name: str, seed: int = 1, n: int | None = None) -> tuple[np
     cfg = dict(LIVE_CONFIGS[name])
     if n is not None:
         cfg["n"] = int(n)
-    pos = globals()[cfg["model"]](cfg["n"], seed)
-    vel = isotropic_velocities(pos, cfg["model"], seed + 1000)
+    if cfg["model"] == "m31_like":
+        pos, comp = m31_like(cfg["n"], seed, components=True)
+        vel = m31_velocities(pos, comp, seed + 1000)
+    else:
+        pos = globals()[cfg["model"]](cfg["n"], seed)
+        vel = isotropic_velocities(pos, cfg["model"], seed + 1000)
     cfg["name"] = name
     cfg["seed"] = seed
     return pos, vel, cfg
