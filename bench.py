@@ -2,7 +2,7 @@
 """bench.py -- whole-hot-path benchmark of the B200-native GOTHIC block-step cycle (driver contract).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME] [--n N]
-    python bench.py --workload nfw_2p22_live | plummer_2p20_live | nfw_2p24_live      (live block stepping only, see measure_live)
+    python bench.py --workload nfw_2p22_live | plummer_2p20_live | nfw_2p24_live | m31_2p24_live      (live block stepping only, see measure_live)
 
 A "step" is one full block-step CYCLE of the workload (BASELINE.json configs[2], NFW sphere N = 2^24 by default):
     gothic_build_tree                                  (B1-B6: bbox, keys, sort, gather, nodes, moments)
@@ -144,23 +144,31 @@ def _sample_ranges(n_groups: int, want: int, pieces: int):
     return out
 
 
-def oracle_cycle_sample(oracle, tree, cfg, r_crit: float, ranges, G: int = 32):
-    """The oracle's share of one step on the sampled i-groups: |a_old| from its own opening-angle bootstrap (R7), block
-    levels of the sampled particles (oracle.levels), then step() = the acceleration-MAC walk of every substep's active set.
+def oracle_bootstrap(oracle, tree, cfg):
+    """|a_old| and the block levels of the FULL particle set from the oracle's own opening-angle bootstrap (R7, R6), so that a
+    sample of i-groups sees the same cycle (finest level, number of substeps) as the whole system does.  Untimed set-up.
+    Returns (aold, level or None, n_substeps)."""
+    n, eps = cfg["n"], cfg["eps"]
+    o, _ = oracle.walk_tree(tree, eps=eps, mac_kind=1, mac_param=THETA_BOOTSTRAP)
+    aold = np.linalg.norm(o[:, :3], axis=1).astype(np.float32)
+    if not cfg["block"]:
+        return aold, None, 1
+    lev, _, n_lev = oracle.levels(o.astype(np.float32), eps, ETA, MAX_LEVELS)
+    return aold, lev, 1 << (n_lev - 1)
+
+
+def oracle_cycle_sample(oracle, tree, cfg, r_crit: float, ranges, boot, G: int = 32):
+    """The oracle's share of one step on the sampled i-groups: step() = the acceleration-MAC walk of every substep's active set among
+    the sampled particles, levels and |a_old| taken from the full set's bootstrap (`boot` = oracle_bootstrap's result).
     Returns (step, n_substeps); step() returns the interactions it evaluated."""
     n, eps, dacc = cfg["n"], cfg["eps"], cfg["delta_acc"]
-    aold = np.ones(n, np.float32)
-    acc = np.zeros((n, 4), np.float32)
-    for lo, hi in ranges:
-        o, _ = oracle.walk_tree(tree, eps=eps, mac_kind=1, mac_param=THETA_BOOTSTRAP, group_range=(lo, hi))
-        acc[lo * G:hi * G] = o[lo * G:hi * G]
-        aold[lo * G:hi * G] = np.linalg.norm(o[lo * G:hi * G, :3], axis=1).astype(np.float32)
+    aold, lev_all, n_sub = boot
     actives = [None]
     if cfg["block"]:
         sel = np.concatenate([np.arange(lo * G, min(n, hi * G), dtype=np.uint32) for lo, hi in ranges])
-        lev, _, n_lev = oracle.levels(acc[sel], eps, ETA, MAX_LEVELS)
+        lev = lev_all[sel]
         actives = []
-        for s in range(1, (1 << (n_lev - 1)) + 1):
+        for s in range(1, n_sub + 1):
             ctz = (s & -s).bit_length() - 1
             actives.append(np.ascontiguousarray(sel[lev <= ctz]))
 
@@ -197,7 +205,10 @@ def run_reference(args, rank: int, world: int):
     n_groups = (n + 31) // 32
     cores = oracle.num_threads()
     ranges = _sample_ranges(n_groups, args.ref_groups, 8)
-    step, n_sub = oracle_cycle_sample(oracle, tree, cfg, r_crit, ranges)
+    t0 = time.time()
+    boot = oracle_bootstrap(oracle, tree, cfg)
+    t_boot = time.time() - t0
+    step, n_sub = oracle_cycle_sample(oracle, tree, cfg, r_crit, ranges, boot)
     for _ in range(args.warmup):
         step()
     t0 = time.time()
@@ -207,14 +218,15 @@ def run_reference(args, rank: int, world: int):
     dt = time.time() - t0
     val = inter / dt
     sample = (f"{sum(hi - lo for lo, hi in ranges)} of {n_groups} i-groups (8 evenly spaced runs), all {n_sub} substeps of the block cycle, "
-              f"fp64 accumulation, {inter // max(args.steps, 1)} interactions per step; oracle tree build {t_build:.1f} s (untimed)")
+              f"levels and |a_old| from the oracle's bootstrap of all {n} particles, fp64 accumulation, {inter // max(args.steps, 1)} interactions per step; "
+              f"oracle tree build {t_build:.1f} s and bootstrap {t_boot:.1f} s (untimed)")
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": 1e3 * dt / max(args.steps, 1), "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic", "config": {"workload": args.workload, "n": n, "eps": eps, "delta_acc": dacc, "r_crit": r_crit, "seed": args.seed},
             "reference_scope": REFERENCE_SCOPE,
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-            "gpu_launches": 0, "setup_s": {"generate": t_gen, "oracle_build": t_build}}
+            "gpu_launches": 0, "setup_s": {"generate": t_gen, "oracle_build": t_build, "oracle_bootstrap": t_boot}}
     print(json.dumps(line), flush=True)
 
 
@@ -227,9 +239,12 @@ def cpu_baseline(pos, cfg, r_crit: float, budget_s: float = 15.0) -> dict:
     t_build = time.time() - t0
     n_groups = (n + 31) // 32
     cores = oracle.num_threads()
+    t0 = time.time()
+    boot = oracle_bootstrap(oracle, tree, cfg)
+    t_boot = time.time() - t0
 
     def run(ranges):
-        step, n_sub = oracle_cycle_sample(oracle, tree, cfg, r_crit, ranges)
+        step, n_sub = oracle_cycle_sample(oracle, tree, cfg, r_crit, ranges, boot)
         t0 = time.time()
         cnt = step()
         return cnt, time.time() - t0, n_sub
@@ -237,14 +252,15 @@ def cpu_baseline(pos, cfg, r_crit: float, budget_s: float = 15.0) -> dict:
     probe = _sample_ranges(n_groups, 64 * cores, 8)
     t0 = time.time()
     cnt, dt, n_sub = run(probe)
-    t_probe = time.time() - t0          # bootstrap + levels + timed walks
+    t_probe = time.time() - t0
     want = int(sum(hi - lo for lo, hi in probe) * budget_s / max(t_probe, 1e-3))
     ranges = _sample_ranges(n_groups, want, 8)
     cnt, dt, n_sub = run(ranges)
     ng = sum(hi - lo for lo, hi in ranges)
     return {"value": cnt / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": f"{ng} of {n_groups} i-groups (8 evenly spaced runs), all {n_sub} substeps of the block cycle, fp64 accumulation, {cnt} interactions in "
-                      f"{dt:.2f} s; oracle tree build at full N took {t_build:.1f} s (not in the rate)",
+            "sample": f"{ng} of {n_groups} i-groups (8 evenly spaced runs), all {n_sub} substeps of the block cycle (levels and |a_old| from the oracle's bootstrap of "
+                      f"all {n} particles), fp64 accumulation, {cnt} interactions in {dt:.2f} s; oracle tree build at full N took {t_build:.1f} s, the bootstrap "
+                      f"{t_boot:.1f} s (not in the rate)",
             "scope": REFERENCE_SCOPE}
 
 
@@ -459,31 +475,46 @@ def measure_sweep(torch, W, B, dev, alu_peak: float, seed: int, reps: int = 3) -
     return {"n": n, "eps": eps, "r_crit": r_crit, "reps": reps, "timing": "best of reps, CUDA events around gothic_walk_tree (group marking included)", "points": points}
 
 
-def measure_live(torch, W, B, workload: str, *, seed: int, n, dev, alu_peak: float, intervals=(1, 2, 4, 12, "cycle"), cycles: int = 2) -> dict:
+def measure_live(torch, W, B, workload: str, *, seed: int, n, dev, alu_peak: float, intervals=(1, 2, 4, 12, "cycle", "auto"), cycles: int = 2) -> dict:
     """The paper's actual time-to-solution loop with MOVING particles through gothic_live_step: per block
     step predict all -> rebuild (every k-th step) or moments refresh -> active list -> walk -> correct with level migration, state on the
     device in tree order.  For each rebuild interval k: one warm-up cycle, then `cycles` block cycles timed with CUDA events
-    (seconds per block step), then one more cycle replayed with the interaction counter read after every step (separate run)."""
+    (seconds per block step), then one more cycle replayed with the interaction counter read after every step (separate run).
+    k = "auto": the rebuild decision of every step comes from paper_1610_07279_b200.tuner.RebuildTuner (eq. 8-12 in the
+    form "rebuild when the walk time lost to the tree's age has reached t_make"), fed with the step's own CUDA-event times
+    (gothic_live_timing: one event wait and a 4-byte read-back per step, inside the timed region); two warm-up cycles instead of one."""
+    from paper_1610_07279_b200.tuner import RebuildTuner
     pos_np, vel_np, cfg = W.make_live_config(workload, seed=seed, n=n)
     n, eps, dacc, r_crit = cfg["n"], cfg["eps"], cfg["delta_acc"], cfg["r_crit"]
     pos, vel = torch.from_numpy(pos_np).to(dev), torch.from_numpy(vel_np).to(dev)
     out = {"workload": workload, "n": n, "eps": eps, "delta_acc": dacc, "r_crit": r_crit, "eta": ETA, "max_levels": MAX_LEVELS, "cycles_timed": cycles,
-           "velocities": "isotropic Gaussian, Jeans dispersion of the truncated profile (workloads.isotropic_velocities)", "rebuild_every": {}}
+           "velocities": ("stand-in: Jeans dispersion of the spherically averaged total profile for halo and bulge, circular speed + 15 % dispersion for the disk "
+                          "(workloads.m31_velocities)") if cfg["model"] == "m31_like" else "isotropic Gaussian, Jeans dispersion of the truncated profile (workloads.isotropic_velocities)", "rebuild_every": {}}
     for k in intervals:
         g = B.Gothic(n, group_size=cfg["group_size"])
         g.live_init(pos, vel, eps=eps, eta=ETA, max_levels=MAX_LEVELS, theta_boot=THETA_BOOTSTRAP)
+        tuner = RebuildTuner() if k == "auto" else None
 
         def run_cycle(counter=None, log=None):
             st = g.live_get(arrays=False)
             for s in range(st["n_substeps"]):
-                rebuild = (s == 0) if k == "cycle" else (st["steps"] + s + 1) % k == 0      # the k-th step of every k: with k = 2, 4 the even (populous) substeps get the fresh tree
+                if tuner is not None:
+                    rebuild = tuner.want_rebuild(s + 1)
+                elif k == "cycle":
+                    rebuild = s == 0
+                else:
+                    rebuild = (st["steps"] + s + 1) % k == 0      # the k-th step of every k: with k = 2, 4 the even (populous) substeps get the fresh tree
                 g.live_step(delta_acc=dacc, r_crit=r_crit, rebuild=rebuild, n_interactions=counter)
+                if tuner is not None:
+                    tuner.observe(s + 1, rebuild, *g.live_timing())
                 if log is not None:
                     now = g.live_get(arrays="n_active")
                     log.append((s + 1, int(now["steps_since_rebuild"]), int(now["n_active"].item()), int(counter.item())))
             return st["n_substeps"]
 
         run_cycle()                       # warm-up
+        if tuner is not None:
+            run_cycle()
         g.check()
         launches0 = g.launch_count()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -506,8 +537,12 @@ def measure_live(torch, W, B, workload: str, *, seed: int, n, dev, alu_peak: flo
         out["rebuild_every"][str(k)] = {
             "sec_per_block_step": ms * 1e-3 / steps, "ms_per_cycle": ms / cycles, "block_steps_timed": steps, "n_substeps_last_cycle": n_sub,
             "interactions_per_cycle": total, "interactions_per_s": total * cycles / (ms * 1e-3) if steps == n_sub * cycles else None,
+            "count_from": "replay cycle: the interactions of ONE later, untimed cycle (PAPER.md:331), scaled to the timed cycles; approximate, the particles have moved on",
             "gpu_launches_per_step": launches / steps,
             "steps": [{"substep": a, "steps_since_rebuild": b, "n_active": c, "interactions": i} for (a, b, c, _), i in zip(log, inter)]}
+        if tuner is not None:
+            out["rebuild_every"][str(k)]["tuner"] = {"rule": "rebuild when the walk time lost since the last rebuild >= t_make (eq. 8-12, PAPER.md:138-175)",
+                                                     "t_make_ms": tuner.t_make, "intervals": tuner.intervals()[-32:]}
         g.close()
     return out
 
@@ -566,7 +601,9 @@ def run_ours(args, rank: int, world: int, local_rank: int):
         alu_peak = props.multi_processor_count * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12      # TFLOP/s, DESIGN.md "Rooflines"
         achieved = walk_rate * FLOP_PER_INTERACTION / 1e12
         traffic, traffic_src = _walk_traffic(args.workload) if args.n is None else (None, None)
-        build_bytes = n * 309 + 0.24 * n * 150
+        # per particle: 309 B with the method's eight LSD passes (8 x 24 B); as run the sort is five passes + the fix-up scan (5 x 24 + 12 B): 249 B
+        build_bytes_8pass = n * 309 + 0.24 * n * 150
+        build_bytes = n * 249 + 0.24 * n * 150
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
             "ms_per_step": total_ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -598,9 +635,12 @@ def run_ours(args, rank: int, world: int, local_rank: int):
                          "peak_source": f"derived: {props.multi_processor_count} SM x 128 FP32 lanes x 2 flop x {peaks['sm_max_mhz']:.0f} MHz "
                                         f"(clock from MEASURED_PEAKS.json, {peaks['source']})"},
             # the HBM-bound part: algorithmic bytes of one build (bbox 16, keys 16 + 8, histogram 8, sort passes x 2 x 12,
-            # gather 4 + 16 + 16, node events 2 x 8 B per particle; moments 16 + 16 + 4 + 1 B per particle and ~150 B per node)
+            # gather 4 + 16 + 16, node events 2 x 8 B per particle; moments 16 + 16 + 4 + 1 B per particle and ~150 B per node); `frac` counts the
+            # five sort passes + fix-up scan that run, `frac_8pass` what the same build would move with the plain eight-pass LSD sort
             "build_roofline": {"bound": "hbm", "achieved": build_bytes / (stage_ms["build"] / K * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
                                "unit": "GB/s", "frac": build_bytes / (stage_ms["build"] / K * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                               "bytes_per_particle": 249, "sort": "as run: 5 one-sweep passes + fix-up scan",
+                               "frac_8pass": build_bytes_8pass / (stage_ms["build"] / K * 1e-3) / 1e9 / peaks["hbm_gbs"],
                                "ms": stage_ms["build"] / K, "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peaks['source']})"},
             "clocks": m["clocks"],
             "gpu_launches": m["launches"],
@@ -622,7 +662,9 @@ def run_ours(args, rank: int, world: int, local_rank: int):
             others["nfw_2p22_sweep"] = measure_sweep(torch, W, B, dev, alu_peak, args.seed)
             line["other_configs"] = others
             # the same sphere with moving particles: predict -> rebuild / refresh -> walk -> correct (gothic_live_step), SURVEY.md 8f row 1
-            line["live"] = measure_live(torch, W, B, "nfw_2p24_live", seed=args.seed, n=None, dev=dev, alu_peak=alu_peak, intervals=(1, 2, 4, "cycle"), cycles=2)
+            line["live"] = measure_live(torch, W, B, "nfw_2p24_live", seed=args.seed, n=None, dev=dev, alu_peak=alu_peak, intervals=(1, 2, 4, "cycle", "auto"), cycles=2)
+            # and the paper's headline model, 64 substeps per cycle: where the fixed per-step costs weigh most
+            line["live_m31"] = measure_live(torch, W, B, "m31_2p24_live", seed=args.seed, n=None, dev=dev, alu_peak=alu_peak, intervals=(1, 2, 4, "auto"), cycles=1)
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(m["pos_np"], cfg, r_crit, args.cpu_budget)
         print(json.dumps(line), flush=True)

@@ -235,6 +235,16 @@ int gothic_live_init(gothic_ctx *ctx, const float *pos_m, const float *vel, uint
 int gothic_live_step(gothic_ctx *ctx, float delta_acc, float r_crit, int rebuild, unsigned long long *n_interactions, void *stream);
 int gothic_live_get(gothic_ctx *ctx, gothic_live_state *out);
 
+/* Device times of the LAST gothic_live_step, for a caller that tunes the rebuild interval from timings as the paper does
+ * (eq. 8-12: t_make against the growth of t_walk).  Every step records three CUDA events on its stream; this call
+ * waits for the last of them (it synchronises with that step's walk, nothing else) and returns
+ *   ms_host[0]  HOST out: the tree stage: predict + rebuild + state re-ordering on a rebuild step, predict + moments refresh otherwise;
+ *   ms_host[1]  HOST out: active list + walk;
+ *   n_active_host  HOST out, may be NULL: the step's number of active particles (a 4-byte read-back).
+ * A step whose active list came back at the end of a cycle is timed like any other (the cycle's level pass is not in either figure).
+ * Errors: GOTHIC_ERR_STATE before the first successful step of a live run. */
+int gothic_live_timing(gothic_ctx *ctx, float *ms_host, uint32_t *n_active_host);
+
 /* Active list of one substep for callers that must not allocate device memory.
  *
  * Who this is for.  Every other compute call needs a gothic_ctx, and gothic_create sizes and cudaMallocs its buffers.  That does

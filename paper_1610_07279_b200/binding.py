@@ -21,7 +21,7 @@ EXPORTS = [
     "gothic_create", "gothic_destroy", "gothic_strerror", "gothic_last_cuda_error", "gothic_build_tree",
     "gothic_update_moments", "gothic_walk_tree", "gothic_set_timesteps", "gothic_get_tree_view", "gothic_check",
     "gothic_gravity_host", "gothic_block_cycle_host", "gothic_launch_count", "gothic_predict", "gothic_correct", "gothic_set_ball",
-    "gothic_live_init", "gothic_live_step", "gothic_live_get", "gothic_active_list_static",
+    "gothic_live_init", "gothic_live_step", "gothic_live_get", "gothic_live_timing", "gothic_active_list_static",
 ]
 STATIC_ACTIVE_MAX_N = 1 << 26     # GOTHIC_STATIC_ACTIVE_MAX_N of include/gothic.h
 
@@ -94,6 +94,8 @@ def load_library():
     L.gothic_live_step.argtypes = [vp, f32, f32, i32, vp, vp]
     L.gothic_live_get.restype = i32
     L.gothic_live_get.argtypes = [vp, C.POINTER(LiveStateStruct)]
+    L.gothic_live_timing.restype = i32
+    L.gothic_live_timing.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(C.c_uint32)]
     L.gothic_active_list_static.restype = i32
     L.gothic_active_list_static.argtypes = [vp, u32, u32, vp, vp, vp]
     L.gothic_launch_count.restype = C.c_ulonglong
@@ -253,6 +255,13 @@ class Gothic:
 
     def live_step(self, *, delta_acc: float, r_crit: float = float("inf"), rebuild: bool = False, n_interactions: torch.Tensor | None = None):
         self._chk(self._L.gothic_live_step(self._ctx, float(delta_acc), float(r_crit), int(bool(rebuild)), _ptr(n_interactions, torch.int64), _stream()))
+
+    def live_timing(self) -> tuple[float, float, int]:
+        """(tree stage ms, active list + walk ms, n_active) of the last live_step, from the step's own CUDA events; waits for that step."""
+        ms = (C.c_float * 2)()
+        na = C.c_uint32(0)
+        self._chk(self._L.gothic_live_timing(self._ctx, ms, C.byref(na)))
+        return float(ms[0]), float(ms[1]), int(na.value)
 
     def live_get(self, arrays: bool | str = True) -> dict:
         """The clock of the live run and (arrays=True) copies of its state rows in tree order (tests, diagnostics); arrays="n_active": only the

@@ -109,6 +109,8 @@ struct gothic_live {
     int e_min, n_levels;
     int key_kind, n_leaf, max_levels;
     float eps, eta;
+    cudaEvent_t ev[3];                        // recorded by every step: start, after the tree stage, after the walk (gothic_live_timing)
+    bool timed;                               // the last step recorded all three
     bool ready;                               // set at the end of gothic_live_init, cleared by any stage that fails: the rows may then be half-way through a step
     unsigned long long tree_gen;              // c->tree_gen after the live run's own last build
 };
@@ -125,6 +127,8 @@ void gothic_live_free(gothic_ctx *c)
     void *ptrs[] = {L->pred, L->acc_new, L->active, L->n_active, L->info_dev};
     for (void *p : ptrs)
         if (p) cudaFree(p);
+    for (cudaEvent_t e : L->ev)
+        if (e) cudaEventDestroy(e);
     delete L;
     c->live = nullptr;
 }
@@ -164,6 +168,8 @@ int live_step_stages(gothic_ctx *c, gothic_live *L, float delta_acc, float r_cri
     int rc;
     const uint32_t t_next = L->t_now + 1u;
     int k = L->cur;
+    L->timed = false;
+    GOTHIC_CUDA_OK(c, cudaEventRecord(L->ev[0], s));
     if (rebuild) {
         // predicted positions in the old order -> new tree (whose gathered copy is the prediction in the new order) -> rows re-ordered
         k_predict<<<grid, TPB, 0, s>>>(L->pos[k], L->vel[k], L->acc[k], L->t_last[k], t_next, dt_unit, n, L->pred);
@@ -182,10 +188,13 @@ int live_step_stages(gothic_ctx *c, gothic_live *L, float delta_acc, float r_cri
         if ((rc = gothic_stage_moments(c, s)) != GOTHIC_OK) return rc;
         L->steps_since_rebuild += 1u;
     }
+    GOTHIC_CUDA_OK(c, cudaEventRecord(L->ev[1], s));
     const float cconst = timestep_constant(L->eps, L->eta);
     if ((rc = gothic_stage_timesteps(c, nullptr, n, cconst, L->max_levels, t_next, L->level[k], L->active, L->n_active, nullptr, s)) != GOTHIC_OK) return rc;
     if ((rc = gothic_stage_walk(c, L->active, 0, L->n_active, L->eps, GOTHIC_MAC_ACCELERATION, delta_acc, r_crit, L->amag[k], L->acc_new, L->amag[k],
                                 n_interactions, s)) != GOTHIC_OK) return rc;
+    GOTHIC_CUDA_OK(c, cudaEventRecord(L->ev[2], s));
+    L->timed = true;
     int cgrid = (int)grid;
     if (cgrid > c->num_sms * 16) cgrid = c->num_sms * 16;
     k_correct<<<cgrid, TPB, 0, s>>>(L->active, 0, L->n_active, c->pos_sorted, L->acc_new, t_next, dt_unit, L->pos[k], L->vel[k], L->acc[k], L->t_last[k],
@@ -256,6 +265,8 @@ int gothic_live_init(gothic_ctx *c, const float *pos_m, const float *vel, uint32
     }
     A(L->pred, float4, n); A(L->acc_new, float4, n); A(L->active, uint32_t, n); A(L->n_active, uint32_t, 1); A(L->info_dev, int32_t, 2);
 #undef A
+    for (int k = 0; k < 3; k++)
+        if (e == cudaSuccess) e = cudaEventCreate(&L->ev[k]);
     if (e != cudaSuccess) { c->last_err = e; gothic_live_free(c); return GOTHIC_ERR_CUDA; }
     int rc = gothic_build_tree(c, pos_m, n, key_kind, n_leaf, stream);
     if (rc != GOTHIC_OK) return rc;
@@ -287,6 +298,18 @@ int gothic_live_step(gothic_ctx *c, float delta_acc, float r_crit, int rebuild, 
     const int rc = live_step_stages(c, L, delta_acc, r_crit, rebuild, n_interactions, stream);
     if (rc != GOTHIC_OK) L->ready = false;       // gothic_live_init starts over
     return rc;
+}
+
+int gothic_live_timing(gothic_ctx *c, float *ms_host, uint32_t *n_active_host)
+{
+    if (!c || !ms_host) return GOTHIC_ERR_ARG;
+    gothic_live *L = c->live;
+    if (!L || !L->ready || !L->timed) return GOTHIC_ERR_STATE;
+    GOTHIC_CUDA_OK(c, cudaEventSynchronize(L->ev[2]));
+    GOTHIC_CUDA_OK(c, cudaEventElapsedTime(ms_host + 0, L->ev[0], L->ev[1]));
+    GOTHIC_CUDA_OK(c, cudaEventElapsedTime(ms_host + 1, L->ev[1], L->ev[2]));
+    if (n_active_host) GOTHIC_CUDA_OK(c, cudaMemcpy(n_active_host, L->n_active, sizeof(uint32_t), cudaMemcpyDeviceToHost));
+    return GOTHIC_OK;
 }
 
 int gothic_live_get(gothic_ctx *c, gothic_live_state *out)

@@ -129,6 +129,39 @@ def test_live_step_refuses_a_tree_that_is_not_its_own():
     g.close()
 
 
+def test_live_timing_feeds_the_rebuild_tuner():
+    """gothic_live_timing returns the last step's stage times and active count; the host-side tuner (eq. 8-12) drives the rebuild flag
+    from them.  The rebuild flag changes no result a tree-independent check can see: the active counts of the cycle are those of a run
+    with a fixed interval, since levels depend on accelerations only to within the MAC's error -- so only sanity is asserted here."""
+    from gpu_util import dev
+    from paper_1610_07279_b200.binding import Gothic, GothicError
+    from paper_1610_07279_b200.tuner import RebuildTuner
+    n, eps = 50000, 1.0 / 64
+    pos = W.plummer(n, seed=31)
+    vel = W.isotropic_velocities(pos, "plummer", seed=32)
+    g = Gothic(n)
+    g.live_init(dev(pos), dev(vel), eps=eps, eta=0.25, max_levels=5, theta_boot=0.5)
+    with pytest.raises(GothicError, match="-2"):
+        g.live_timing()                                       # no step yet
+    tuner = RebuildTuner(max_age=6)
+    for cycle in range(3):
+        st = g.live_get(arrays=False)
+        for s in range(st["n_substeps"]):
+            rebuild = tuner.want_rebuild(s + 1)
+            g.live_step(delta_acc=2.0 ** -8, r_crit=0.5, rebuild=rebuild)
+            tree_ms, walk_ms, n_active = g.live_timing()
+            assert 0.0 < tree_ms < 1e3 and 0.0 <= walk_ms < 1e3
+            assert n_active == int(g.live_get(arrays="n_active")["n_active"].item()) and 0 <= n_active <= n
+            assert g.live_get(arrays=False)["steps_since_rebuild"] == (0 if rebuild else tuner.age + 1)
+            tuner.observe(s + 1, rebuild, tree_ms, walk_ms, n_active)
+        assert n_active == n                                  # the last substep of a cycle has everybody active
+    g.check()
+    assert tuner.t_make is not None and tuner.t_make >= 0.0
+    iv = tuner.intervals()
+    assert len(iv) >= 2 and max(iv) <= 6
+    g.close()
+
+
 def test_live_free_running_vs_oracle_only(oracle):
     """Nothing of the CUDA path on the reference side: the oracle integrates the same initial conditions with its own trees, its own
     moments and double-precision sums (tree rebuilt every second step on both sides).  After one full cycle positions and velocities
